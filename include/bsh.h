@@ -1,0 +1,160 @@
+/*
+ * bsh.h -- C ABI of the B200-native BinarySkyHough hot path (Covas & Sintes, arXiv:1904.04873).
+ *
+ * Citations are lines of /root/reference/PAPER.md ("L123") with the section / equation they fall in, or DESIGN.md
+ * readings ("R-5").  The library computes, for every template of a sky patch x template grid,
+ *
+ *   peakgram   bit[i][k] = rho[i][k] > rho_th                                   L176 (sec. IV.A), rho_th = 1.6
+ *   track      k_i = round((f(t_i) - f_slab_start) T),                          BASELINE.json north_star
+ *              f(t) = f0 [1 + v(t).n/c - a_p Omega cos(Omega (t - t_asc))]      L102 Eq. (15), Omega = 2 pi / P (L61)
+ *   stage 1    n = sum_i bit[i][k_i],  n_w = sum_i w_i bit[i][k_i]              L223 (sec. IV.C) "number count"
+ *   toplist    the topk templates of the patch by the stage-1 statistic         L217, L225-L229
+ *   stage 2    P = sum_i w_i rho[i][k_i] along the same track                   L227 Eq. (26)
+ *
+ * Conventions
+ *   - Every function returns int: BSH_OK (0) or a negative error code.  Nothing throws; bsh_last_error(ctx) returns a
+ *     description of the last failure on that context (valid until the next call on it).
+ *   - Pointer prefixes:  d_ = DEVICE memory owned by the caller, never freed or retained by the library beyond the
+ *     call unless stated;  h_ = HOST memory, read (or written) during the call only.
+ *   - All device work is enqueued on the CUDA stream given to bsh_create().  Functions documented "asynchronous"
+ *     return before the work completes; the caller synchronises that stream before reading results.
+ *   - There is no CPU fallback: without a CUDA device bsh_create() fails with BSH_ECUDA.
+ *   - Template linear index (R-11): ((((pix * n_ap + ia) * n_P + ip) * n_tasc + it) * n_f0 + j, f0 fastest.
+ *   - Ordering everywhere: (statistic descending, template index ascending).
+ */
+#ifndef BSH_H_
+#define BSH_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BSH_OK        0
+#define BSH_EINVAL   -1   /* bad size / null pointer / inconsistent arguments (nothing was launched)            */
+#define BSH_ENOMEM   -2   /* device or host allocation failed                                                    */
+#define BSH_ECUDA    -3   /* a CUDA runtime call or kernel failed (message in bsh_last_error)                    */
+#define BSH_ESMALL   -4   /* an output buffer is too small (e.g. words_per_row * 32 < n_bins)                    */
+#define BSH_ESTATE   -5   /* call order violated (e.g. bsh_stage1_collect without bsh_stage1_launch)             */
+
+/* mode bits for stage 1 */
+#define BSH_UNWEIGHTED 0  /* rank by the integer number count n                                   (L223)         */
+#define BSH_WEIGHTED   1  /* rank by n_w = sum w_i bit, FP32 accumulation in SFT order            (L223, Eq. 22) */
+#define BSH_NAIVE      16 /* diagnostic: one thread per template, one track evaluation per (template, SFT), global-
+                             memory gathers.  Same results; exists to cross-check the tiled kernels at full size. */
+
+typedef struct bsh_ctx bsh_ctx;
+
+/* One SFT set.  Stage 1 and stage 2 may be given different sets (the paper's stage 2 adds half-overlapped SFTs,
+ * L233); all five BASELINE.json configs use the same set for both. */
+typedef struct {
+    int32_t       n_sft;         /* N >= 1                                                                       */
+    double        t_sft;         /* T = T_c, seconds; the bin width is 1/T (Eq. 33)                        */
+    const double *h_t_mid;       /* [N] SFT mid-times in seconds relative to any reference epoch (R-2); the same  */
+                                 /*     epoch as t_search_mid.  Keep |Omega t| moderate (epoch near the data).    */
+    const double *h_v_over_c;    /* [N][3] detector velocity / c at t_mid, equatorial frame; one row per SFT, so  */
+                                 /*     several detectors are simply more rows                                    */
+    const float  *d_w;           /* [N] per-SFT weights (Eq. 22), caller-normalised (R-9); NULL = all 1     */
+    int64_t       k_slab0;       /* absolute frequency-bin index (f * T) of column 0 of the slab                  */
+    int32_t       n_bins;        /* K = slab columns                                                              */
+    double        t_search_mid;  /* t_mid of Eq. (35) (L305)                                                      */
+} bsh_sfts;
+
+/* One sky patch x template grid. */
+typedef struct {
+    int32_t n_pix;  const double *h_alpha, *h_delta;  /* [n_pix] right ascension / declination, radians           */
+    int64_t k_band0;                                  /* f0_j = (k_band0 + j) / T, j = 0 .. n_f0-1 (R-3);          */
+    int32_t n_f0;                                     /*   requires k_band0 >= k_slab0                             */
+    int32_t n_ap;   const double *h_ap;               /* [n_ap]  projected semi-major axis, light-seconds (L70)    */
+    int32_t n_P;    const double *h_P;                /* [n_P]   orbital period, seconds                           */
+    int32_t n_tasc; const double *h_tasc_frac;        /* [n_tasc] t_asc = t_search_mid + frac * P (Eq. 35, R-13)   */
+} bsh_grid;
+
+/* Toplist / candidate record (24 bytes). */
+typedef struct {
+    uint64_t index;    /* template linear index                                                                    */
+    int32_t  count;    /* n   = sum_i bit                    (exact)                                               */
+    float    wcount;   /* n_w = sum_i w_i bit                (FP32; = count when d_w is NULL)                       */
+    float    power;    /* P   = sum_i w_i rho, Eq. (26)      (filled by bsh_stage2_power; 0 before)                */
+    uint32_t flags;    /* bit 0: filled by stage 1; bit 1: power filled                                            */
+} bsh_cand;
+
+/* Diagnostics of the most recent calls on a context (all times in milliseconds, from CUDA events on the stream). */
+typedef struct {
+    float    peakgram_ms;        /* bsh_build_peakgram kernel                                                      */
+    float    stage1_setup_ms;    /* window table, D table, threshold (device side)                                 */
+    float    stage1_kernel_ms;   /* the accumulation kernel(s) of the last bsh_stage1_* (all passes)               */
+    float    stage1_select_ms;   /* candidate sort + toplist rescoring                                             */
+    float    stage2_ms;          /* bsh_stage2_power kernels                                                       */
+    int64_t  n_templates;        /* templates of the last stage-1 call                                             */
+    int64_t  n_accumulations;    /* n_templates * n_sft                                                            */
+    int64_t  n_candidates;       /* templates that passed the in-kernel threshold                                  */
+    double   threshold;          /* final in-kernel threshold (count or weighted count)                            */
+    int32_t  n_passes;           /* accumulation passes (1 unless the threshold had to be moved)                   */
+    int32_t  kernel_variant;     /* words * 100 + pixels_per_thread * 10 + clamp                                   */
+    int32_t  threads_per_block;  /* of the accumulation kernel                                                     */
+    int32_t  grid_blocks;        /* of the accumulation kernel                                                     */
+    int64_t  launches;           /* kernels launched by this context since creation                                */
+    float    host_tables_ms;     /* host time spent building cos/sin tables in the last call (0 when cached)       */
+} bsh_stats;
+
+/* Create a context bound to `device` and to `cuda_stream` (a cudaStream_t; NULL = legacy default stream).
+ * The context owns scratch memory (tables, candidate buffer), grown on demand and freed by bsh_destroy. */
+int bsh_create(bsh_ctx **out, int device, void *cuda_stream);
+int bsh_destroy(bsh_ctx *ctx);
+const char *bsh_last_error(const bsh_ctx *ctx);
+int bsh_get_stats(bsh_ctx *ctx, bsh_stats *out);     /* synchronises the stream to read event timers */
+int bsh_version(void);
+
+/* Peakgram (L176): d_peak[i][k >> 5] bit (k & 31) = (d_rho[i * rho_row_stride + k] > rho_th), strict '>' in FP32,
+ * NaN -> 0 (R-8); pad bits of each row are zero.  d_rho: [n_sft][rho_row_stride] FP32, rho_row_stride >= n_bins
+ * (elements).  d_peak: [n_sft][words_per_row] uint32, words_per_row >= ceil(n_bins / 32) (else BSH_ESMALL); words
+ * beyond ceil(n_bins / 32) are zeroed.  Asynchronous. */
+int bsh_build_peakgram(bsh_ctx *ctx, const float *d_rho, int32_t n_sft, int32_t n_bins, int64_t rho_row_stride,
+                       float rho_th, uint32_t *d_peak, int32_t words_per_row);
+
+/* Stage 1 (L223, L241-L247): number count of every template of `grid` along its Eq. (15) track through the
+ * peakgram, and the per-patch toplist (L217, L225).
+ *   d_peak          [n_sft][words_per_row] as written by bsh_build_peakgram for this SFT set
+ *   mode            BSH_UNWEIGHTED or BSH_WEIGHTED (needs sfts->d_w), optionally | BSH_NAIVE
+ *   topk            entries wanted, 1 <= topk
+ *   d_top           [topk] records, best first; entries beyond *h_n_top are zeroed
+ *   h_n_top         receives min(topk, n_templates)
+ *   d_counts_full   optional dump of the ranking statistic of EVERY template (int32 counts in BSH_UNWEIGHTED mode,
+ *                   float weighted counts in BSH_WEIGHTED mode), [n_templates]; NULL in production
+ * A track leaving the slab is not an error: that SFT contributes 0 (R-6).
+ * bsh_stage1_hough = bsh_stage1_launch + bsh_stage1_collect; it returns with d_top complete (stream synchronised).
+ * bsh_stage1_launch is asynchronous (no host synchronisation); bsh_stage1_collect synchronises the stream, runs the
+ * selection, and leaves the toplist writes enqueued on the stream (h_n_top is final on return).  Between launch and
+ * collect the caller may enqueue work on OTHER contexts/streams (this is how config 5 overlaps two patches).
+ * The host arrays inside `sfts` and `grid` are read during launch only. */
+int bsh_stage1_hough(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_row, const bsh_sfts *sfts,
+                     const bsh_grid *grid, int32_t mode, int32_t topk, bsh_cand *d_top, int32_t *h_n_top,
+                     void *d_counts_full);
+int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_row, const bsh_sfts *sfts,
+                      const bsh_grid *grid, int32_t mode, int32_t topk, void *d_counts_full);
+int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top);
+
+/* Stage 2 (Eq. 26): power[c] = sum_i w_i rho[i][k_i] along the track of d_cands[c].index over the SFT set
+ * `sfts` (FP32 products, each lane sums every 32nd SFT in order, then a fixed shuffle tree; R-20), written into
+ * d_cands[c].power.  If sort_by_power != 0 the records are then reordered by (power desc, index asc).
+ * d_rho: [n_sft][rho_row_stride] FP32.  Asynchronous. */
+int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, const bsh_sfts *sfts,
+                     const bsh_grid *grid, bsh_cand *d_cands, int32_t n_cands, int32_t sort_by_power);
+
+/* Whole patch from HOST buffers (the end-to-end call): copies h_rho [n_sft][n_bins] and h_w [n_sft] (may be NULL) to
+ * the device, builds the peakgram, runs stage 1 and stage 2 (sorted by power) and copies the toplist back into
+ * h_top [topk].  sfts->d_w is ignored (h_w is used).  Synchronous. */
+int bsh_search_patch_host(bsh_ctx *ctx, const float *h_rho, const float *h_w, float rho_th, const bsh_sfts *sfts,
+                          const bsh_grid *grid, int32_t mode, int32_t topk, bsh_cand *h_top, int32_t *h_n_top);
+
+/* Template index helpers (R-11).  Pure host functions. */
+uint64_t bsh_template_index(const bsh_grid *grid, int32_t pix, int32_t ia, int32_t ip, int32_t it, int32_t j);
+void     bsh_template_decode(const bsh_grid *grid, uint64_t index, int32_t *pix, int32_t *ia, int32_t *ip,
+                             int32_t *it, int32_t *j);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BSH_H_ */

@@ -1,0 +1,201 @@
+"""ctypes binding of include/bsh.h -- argument marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+BSH_UNWEIGHTED, BSH_WEIGHTED, BSH_NAIVE = 0, 1, 16
+
+EXPORTS = ["bsh_version", "bsh_create", "bsh_destroy", "bsh_last_error", "bsh_get_stats", "bsh_build_peakgram",
+           "bsh_stage1_hough", "bsh_stage1_launch", "bsh_stage1_collect", "bsh_stage2_power", "bsh_search_patch_host",
+           "bsh_template_index", "bsh_template_decode"]
+
+# numpy view of bsh_cand (24 bytes)
+CAND_DTYPE = np.dtype([("index", "<u8"), ("count", "<i4"), ("wcount", "<f4"), ("power", "<f4"), ("flags", "<u4")])
+
+
+class BshError(RuntimeError):
+    pass
+
+
+class _Sfts(C.Structure):
+    _fields_ = [("n_sft", C.c_int32), ("t_sft", C.c_double), ("h_t_mid", C.c_void_p), ("h_v_over_c", C.c_void_p),
+                ("d_w", C.c_void_p), ("k_slab0", C.c_int64), ("n_bins", C.c_int32), ("t_search_mid", C.c_double)]
+
+
+class _Grid(C.Structure):
+    _fields_ = [("n_pix", C.c_int32), ("h_alpha", C.c_void_p), ("h_delta", C.c_void_p), ("k_band0", C.c_int64),
+                ("n_f0", C.c_int32), ("n_ap", C.c_int32), ("h_ap", C.c_void_p), ("n_P", C.c_int32), ("h_P", C.c_void_p),
+                ("n_tasc", C.c_int32), ("h_tasc_frac", C.c_void_p)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("peakgram_ms", C.c_float), ("stage1_setup_ms", C.c_float), ("stage1_kernel_ms", C.c_float),
+                ("stage1_select_ms", C.c_float), ("stage2_ms", C.c_float), ("n_templates", C.c_int64),
+                ("n_accumulations", C.c_int64), ("n_candidates", C.c_int64), ("threshold", C.c_double),
+                ("n_passes", C.c_int32), ("kernel_variant", C.c_int32), ("threads_per_block", C.c_int32),
+                ("grid_blocks", C.c_int32), ("launches", C.c_int64), ("host_tables_ms", C.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def library():
+    """Load (building if needed) the in-tree libbsh.so.  Raises if it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.build_library()
+        lib = C.CDLL(path)
+        lib.bsh_last_error.restype = C.c_char_p
+        lib.bsh_template_index.restype = C.c_uint64
+        lib.bsh_template_decode.restype = None
+        for name in EXPORTS:
+            getattr(lib, name)                       # fail loudly on a missing symbol
+        _lib = lib
+    return _lib
+
+
+class _Problem:
+    """Host arrays (kept alive) + the two C structs describing one workload."""
+
+    def __init__(self, wl, d_w=None):
+        f64 = lambda a: np.ascontiguousarray(a, np.float64)
+        self.a = dict(t_mid=f64(wl.t_mid), v=f64(wl.v_over_c), alpha=f64(wl.alpha), delta=f64(wl.delta), ap=f64(wl.ap),
+                      P=f64(wl.P), tf=f64(wl.tasc_frac))
+        a = self.a
+        self.sfts = _Sfts(n_sft=a["t_mid"].shape[0], t_sft=float(wl.t_sft), h_t_mid=a["t_mid"].ctypes.data,
+                          h_v_over_c=a["v"].ctypes.data, d_w=(d_w.data_ptr() if d_w is not None else None),
+                          k_slab0=int(wl.k_slab0), n_bins=int(wl.n_bins), t_search_mid=float(wl.t_search_mid))
+        self.grid = _Grid(n_pix=a["alpha"].shape[0], h_alpha=a["alpha"].ctypes.data, h_delta=a["delta"].ctypes.data,
+                          k_band0=int(wl.k_band0), n_f0=int(wl.n_f0), n_ap=a["ap"].shape[0], h_ap=a["ap"].ctypes.data,
+                          n_P=a["P"].shape[0], h_P=a["P"].ctypes.data, n_tasc=a["tf"].shape[0],
+                          h_tasc_frac=a["tf"].ctypes.data)
+        self.d_w = d_w
+
+
+def template_index(wl, pix, ia, ip, it, j) -> int:
+    return int(library().bsh_template_index(C.byref(_Problem(wl).grid), pix, ia, ip, it, j))
+
+
+def template_decode(wl, index):
+    out = [C.c_int32() for _ in range(5)]
+    library().bsh_template_decode(C.byref(_Problem(wl).grid), C.c_uint64(int(index)), *[C.byref(o) for o in out])
+    return tuple(o.value for o in out)
+
+
+class Context:
+    """One bsh_ctx bound to a torch CUDA device and stream."""
+
+    def __init__(self, device: int = 0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise BshError("no CUDA device: the BinarySkyHough path has no CPU fallback")
+        self.torch = torch
+        self.lib = library()
+        self.device = device
+        torch.cuda.set_device(device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(device)
+        self._ctx = C.c_void_p()
+        rc = self.lib.bsh_create(C.byref(self._ctx), C.c_int(device), C.c_void_p(self.stream.cuda_stream))
+        if rc != 0:
+            raise BshError(f"bsh_create failed ({rc})")
+        self._keep = []
+
+    def close(self):
+        if self._ctx:
+            self.lib.bsh_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != 0:
+            raise BshError(f"bsh error {rc}: {self.lib.bsh_last_error(self._ctx).decode()}")
+
+    # ---- the three calls of the path -------------------------------------------------------------------------------
+    def build_peakgram(self, d_rho, rho_th: float = 1.6, out=None):
+        """d_rho: CUDA float32 [N, K] (row stride = d_rho.stride(0)).  Returns CUDA int32 tensor [N, ceil(K/32)] holding
+        the uint32 bit words."""
+        torch = self.torch
+        assert d_rho.is_cuda and d_rho.dtype == torch.float32 and d_rho.dim() == 2 and d_rho.stride(1) == 1
+        n, k = d_rho.shape
+        wpr = (k + 31) // 32
+        if out is None:
+            out = torch.empty((n, wpr), dtype=torch.int32, device=d_rho.device)
+        self._check(self.lib.bsh_build_peakgram(self._ctx, C.c_void_p(d_rho.data_ptr()), C.c_int32(n), C.c_int32(k),
+                                                C.c_int64(d_rho.stride(0)), C.c_float(rho_th), C.c_void_p(out.data_ptr()),
+                                                C.c_int32(out.shape[1])))
+        return out
+
+    def stage1_launch(self, d_peak, wl, mode=BSH_UNWEIGHTED, topk=None, d_w=None, counts_full=None):
+        pb = _Problem(wl, d_w)
+        topk = int(topk if topk is not None else wl.topk)
+        self._pending = (pb, topk)
+        self._check(self.lib.bsh_stage1_launch(self._ctx, C.c_void_p(d_peak.data_ptr()), C.c_int32(d_peak.shape[1]),
+                                               C.byref(pb.sfts), C.byref(pb.grid), C.c_int32(mode), C.c_int32(topk),
+                                               C.c_void_p(counts_full.data_ptr() if counts_full is not None else None)))
+
+    def stage1_collect(self):
+        torch = self.torch
+        pb, topk = self._pending
+        d_top = torch.empty(topk * CAND_DTYPE.itemsize, dtype=torch.uint8, device=f"cuda:{self.device}")
+        n_top = C.c_int32(0)
+        self._check(self.lib.bsh_stage1_collect(self._ctx, C.c_void_p(d_top.data_ptr()), C.byref(n_top)))
+        return d_top, int(n_top.value)
+
+    def stage1_hough(self, d_peak, wl, mode=BSH_UNWEIGHTED, topk=None, d_w=None, counts_full=None):
+        """Returns (d_top, n_top): d_top is a CUDA uint8 tensor holding topk bsh_cand records (best first)."""
+        torch = self.torch
+        pb = _Problem(wl, d_w)
+        topk = int(topk if topk is not None else wl.topk)
+        d_top = torch.empty(topk * CAND_DTYPE.itemsize, dtype=torch.uint8, device=f"cuda:{self.device}")
+        n_top = C.c_int32(0)
+        self._check(self.lib.bsh_stage1_hough(self._ctx, C.c_void_p(d_peak.data_ptr()), C.c_int32(d_peak.shape[1]),
+                                              C.byref(pb.sfts), C.byref(pb.grid), C.c_int32(mode), C.c_int32(topk),
+                                              C.c_void_p(d_top.data_ptr()), C.byref(n_top),
+                                              C.c_void_p(counts_full.data_ptr() if counts_full is not None else None)))
+        return d_top, int(n_top.value)
+
+    def stage2_power(self, d_rho, wl, d_cands, n_cands: int, d_w=None, sort_by_power: bool = True):
+        pb = _Problem(wl, d_w)
+        self._check(self.lib.bsh_stage2_power(self._ctx, C.c_void_p(d_rho.data_ptr()), C.c_int64(d_rho.stride(0)),
+                                              C.byref(pb.sfts), C.byref(pb.grid), C.c_void_p(d_cands.data_ptr()),
+                                              C.c_int32(n_cands), C.c_int32(int(sort_by_power))))
+        return d_cands
+
+    def search_patch_host(self, rho: np.ndarray, w: Optional[np.ndarray], wl, mode=BSH_UNWEIGHTED, topk=None,
+                          rho_th: float = 1.6, out: Optional[np.ndarray] = None):
+        """End-to-end call on HOST buffers (numpy, ideally pinned): returns (records[topk], n_top)."""
+        topk = int(topk if topk is not None else wl.topk)
+        pb = _Problem(wl, None)
+        if out is None:
+            out = np.zeros(topk, CAND_DTYPE)
+        n_top = C.c_int32(0)
+        wp = None if w is None else C.c_void_p(w.ctypes.data)
+        self._check(self.lib.bsh_search_patch_host(self._ctx, C.c_void_p(rho.ctypes.data), wp, C.c_float(rho_th),
+                                                   C.byref(pb.sfts), C.byref(pb.grid), C.c_int32(mode), C.c_int32(topk),
+                                                   C.c_void_p(out.ctypes.data), C.byref(n_top)))
+        return out, int(n_top.value)
+
+    def stats(self) -> dict:
+        s = Stats()
+        self._check(self.lib.bsh_get_stats(self._ctx, C.byref(s)))
+        return s.as_dict()
+
+    @staticmethod
+    def records(d_top, n=None) -> np.ndarray:
+        """CUDA uint8 record buffer -> numpy structured array."""
+        a = d_top.cpu().numpy().view(CAND_DTYPE)
+        return a if n is None else a[:n]

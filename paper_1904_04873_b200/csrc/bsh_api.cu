@@ -1,0 +1,681 @@
+// bsh_api.cu -- C ABI (include/bsh.h) of the B200-native BinarySkyHough hot path: context, host-side table building
+// (the only place transcendentals are evaluated, R-5), kernel selection and launch, candidate selection.
+// Build: nvcc -O3 -std=c++17 -gencode arch=compute_100a,code=sm_100a -lineinfo -Xcompiler -fPIC,-ffp-contract=off -shared
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <chrono>
+#include <string>
+#include <vector>
+
+#include "../../include/bsh.h"
+#include "bsh_host.hpp"
+#include "bsh_kernels.cuh"
+
+using namespace bsh;
+
+namespace {
+
+constexpr unsigned int kCandCap = 1u << 20;      // candidate buffer entries (16 MB)
+constexpr int kMaxPasses = 12;
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t bytes = 0;
+};
+
+struct TableCache {                   // cos/sin tables of one (SFT set, binary grid); content-addressed
+    bool valid = false;
+    uint64_t stamp = 0;
+    std::vector<double> t_mid, v, P, tasc, ap;
+    double t_sft = 0, t_search_mid = 0;
+    int n_sft = 0, n_pad = 0, n_P = 0, n_tasc = 0, n_ap = 0;
+    DevBuf d_v, d_cs, d_casa, d_A;
+};
+
+struct Pending {                      // state between bsh_stage1_launch and bsh_stage1_collect
+    bool active = false;
+    int mode = 0, topk = 0;
+    void *d_counts_full = nullptr;
+    const uint32_t *d_peak = nullptr;
+    int words_per_row = 0;
+    const float *d_w = nullptr;
+    int cache_slot = 0;
+    int n_sft = 0, n_pad = 0, n_bins = 0, n_pix = 0, n_ap = 0, n_P = 0, n_tasc = 0, n_f0 = 0;
+    int64_t k_band0 = 0, k_slab0 = 0;
+    uint64_t n_templates = 0;
+    bool emit_all = false, clamp = false;
+    int R = 2, NW = 3, HP = 6, n_entries = 0, off_table = 0, s_max = 0, tpb = 256, n_groups = 0, n_aq_tiles = 0;
+    double frac = 0, shift_sigma = 0;
+    int passes = 0;
+};
+
+}  // namespace
+
+struct bsh_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    TableCache cache[2];
+    uint64_t stamp = 0;
+    DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2;
+    DevBuf h_rho, h_w, h_peak, h_top;                  // device staging of bsh_search_patch_host
+    unsigned int *pinned_count = nullptr;
+    cudaEvent_t ev[10] = {};
+    Pending pend;
+    bsh_stats st = {};
+    bool have_pk = false, have_setup = false, have_kernel = false, have_select = false, have_s2 = false;
+    float kernel_ms_extra = 0.f;
+};
+
+namespace {
+
+int fail(bsh_ctx *ctx, int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf;
+    return code;
+}
+
+#define CK(call)                                                                                              \
+    do {                                                                                                      \
+        cudaError_t e_ = (call);                                                                              \
+        if (e_ != cudaSuccess)                                                                                \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? BSH_ENOMEM : BSH_ECUDA, "%s failed: %s (%s:%d)", \
+                        #call, cudaGetErrorString(e_), __FILE__, __LINE__);                                   \
+    } while (0)
+
+int ensure(bsh_ctx *ctx, DevBuf &b, size_t bytes)
+{
+    if (b.bytes >= bytes && b.p) return BSH_OK;
+    if (b.p) {
+        CK(cudaStreamSynchronize(ctx->stream));
+        CK(cudaFree(b.p));
+        b.p = nullptr;
+        b.bytes = 0;
+    }
+    const size_t want = std::max<size_t>(bytes + bytes / 4, 256);
+    CK(cudaMalloc(&b.p, want));
+    b.bytes = want;
+    return BSH_OK;
+}
+
+#define TRY(expr)                  \
+    do {                           \
+        int rc_ = (expr);          \
+        if (rc_ != BSH_OK) return rc_; \
+    } while (0)
+
+inline void count_launch(bsh_ctx *ctx, int n = 1) { ctx->st.launches += n; }
+
+static_assert(kHostChunk == kChunk, "SFT padding granularity");
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Host tables (R-5).  The only transcendental evaluations of the whole path: libm cos/sin of Omega_p t_i and
+// Omega_p t_asc, and of the pixel angles.  Cached by content: a sweep over sky patches reuses them.
+// ---------------------------------------------------------------------------------------------------------------------
+int validate(bsh_ctx *ctx, const bsh_sfts *s, const bsh_grid *g)
+{
+    if (!s || !g) return fail(ctx, BSH_EINVAL, "null sfts/grid");
+    if (s->n_sft < 1 || !(s->t_sft > 0) || !s->h_t_mid || !s->h_v_over_c || s->n_bins < 1)
+        return fail(ctx, BSH_EINVAL, "bad SFT set (n_sft=%d, t_sft=%g, n_bins=%d)", s->n_sft, s->t_sft, s->n_bins);
+    if (g->n_pix < 1 || g->n_f0 < 1 || g->n_ap < 1 || g->n_P < 1 || g->n_tasc < 1 || !g->h_alpha || !g->h_delta ||
+        !g->h_ap || !g->h_P || !g->h_tasc_frac)
+        return fail(ctx, BSH_EINVAL, "bad grid");
+    if (g->k_band0 < s->k_slab0) return fail(ctx, BSH_EINVAL, "k_band0 < k_slab0");
+    if (g->k_band0 - s->k_slab0 > (1 << 24) || g->k_band0 + g->n_f0 >= (1ll << 40))
+        return fail(ctx, BSH_EINVAL, "band offset out of range");
+    for (int p = 0; p < g->n_P; ++p)
+        if (!(g->h_P[p] > 0)) return fail(ctx, BSH_EINVAL, "P[%d] <= 0", p);
+    return BSH_OK;
+}
+
+int get_tables(bsh_ctx *ctx, const bsh_sfts *s, const bsh_grid *g, int *slot_out)
+{
+    const int N = s->n_sft;
+    for (int k = 0; k < 2; ++k) {
+        TableCache &c = ctx->cache[k];
+        if (c.valid && c.n_sft == N && c.n_P == g->n_P && c.n_tasc == g->n_tasc && c.n_ap == g->n_ap &&
+            c.t_sft == s->t_sft && c.t_search_mid == s->t_search_mid &&
+            !memcmp(c.t_mid.data(), s->h_t_mid, sizeof(double) * N) &&
+            !memcmp(c.v.data(), s->h_v_over_c, sizeof(double) * 3 * N) &&
+            !memcmp(c.P.data(), g->h_P, sizeof(double) * g->n_P) &&
+            !memcmp(c.tasc.data(), g->h_tasc_frac, sizeof(double) * g->n_tasc) &&
+            !memcmp(c.ap.data(), g->h_ap, sizeof(double) * g->n_ap)) {
+            c.stamp = ++ctx->stamp;
+            *slot_out = k;
+            ctx->st.host_tables_ms = 0.f;
+            return BSH_OK;
+        }
+    }
+    const auto t0 = std::chrono::steady_clock::now();
+    const int k = (!ctx->cache[0].valid || (ctx->cache[1].valid && ctx->cache[0].stamp < ctx->cache[1].stamp)) ? 0 : 1;
+    TableCache &c = ctx->cache[k];
+    c.valid = false;
+    const int n_pad = pad_sfts(N);
+    c.t_mid.assign(s->h_t_mid, s->h_t_mid + N);
+    c.v.assign(s->h_v_over_c, s->h_v_over_c + 3 * (size_t)N);
+    c.P.assign(g->h_P, g->h_P + g->n_P);
+    c.tasc.assign(g->h_tasc_frac, g->h_tasc_frac + g->n_tasc);
+    c.ap.assign(g->h_ap, g->h_ap + g->n_ap);
+    c.t_sft = s->t_sft;
+    c.t_search_mid = s->t_search_mid;
+    c.n_sft = N; c.n_pad = n_pad; c.n_P = g->n_P; c.n_tasc = g->n_tasc; c.n_ap = g->n_ap;
+
+    std::vector<double> cs, casa, A;
+    build_binary_tables(N, n_pad, s->h_t_mid, s->t_search_mid, g->n_P, g->h_P, g->n_tasc, g->h_tasc_frac, g->n_ap, g->h_ap, cs,
+                        casa, A);
+    TRY(ensure(ctx, c.d_v, sizeof(double) * 3 * (size_t)N));
+    TRY(ensure(ctx, c.d_cs, sizeof(double) * cs.size()));
+    TRY(ensure(ctx, c.d_casa, sizeof(double) * casa.size()));
+    TRY(ensure(ctx, c.d_A, sizeof(double) * A.size()));
+    CK(cudaMemcpyAsync(c.d_v.p, c.v.data(), sizeof(double) * 3 * (size_t)N, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(c.d_cs.p, cs.data(), sizeof(double) * cs.size(), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(c.d_casa.p, casa.data(), sizeof(double) * casa.size(), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(c.d_A.p, A.data(), sizeof(double) * A.size(), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));          // the std::vectors above go out of scope
+    c.valid = true;
+    c.stamp = ++ctx->stamp;
+    *slot_out = k;
+    ctx->st.host_tables_ms =
+        std::chrono::duration<float, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    return BSH_OK;
+}
+
+// pixel unit vectors (host libm) -> device; D table on the device
+int build_dtable(bsh_ctx *ctx, const bsh_grid *g, const TableCache &c, int R, DevBuf &nvec_buf, DevBuf &dtab_buf)
+{
+    std::vector<double> nv;
+    pixel_vectors(g->n_pix, g->h_alpha, g->h_delta, nv);
+    const int n_groups = (g->n_pix + R - 1) / R;
+    TRY(ensure(ctx, nvec_buf, sizeof(double) * nv.size()));
+    TRY(ensure(ctx, dtab_buf, sizeof(double) * (size_t)n_groups * c.n_pad * R));
+    CK(cudaMemcpyAsync(nvec_buf.p, nv.data(), sizeof(double) * nv.size(), cudaMemcpyHostToDevice, ctx->stream));
+    const int64_t total = (int64_t)n_groups * c.n_pad * R;
+    dtable_kernel<<<(unsigned)((total + 255) / 256), 256, 0, ctx->stream>>>(
+        (const double *)c.d_v.p, (const double *)nvec_buf.p, c.n_sft, c.n_pad, g->n_pix, n_groups, R, (double *)dtab_buf.p);
+    count_launch(ctx);
+    CK(cudaGetLastError());
+    return BSH_OK;
+}
+
+TrackTables make_track_tables(const TableCache &c, const bsh_sfts *s, const bsh_grid *g, const double *dtab, int R)
+{
+    TrackTables t;
+    t.cs = (const double2 *)c.d_cs.p;
+    t.dtab = dtab;
+    t.A = (const double *)c.d_A.p;
+    t.casa = (const double2 *)c.d_casa.p;
+    t.n_pad = c.n_pad;
+    t.R = R;
+    t.n_pix = g->n_pix; t.n_ap = g->n_ap; t.n_P = g->n_P; t.n_tasc = g->n_tasc; t.n_f0 = g->n_f0;
+    t.k_band0 = g->k_band0;
+    t.m = (int)(g->k_band0 - s->k_slab0);
+    t.n_bins = s->n_bins;
+    t.n_sft = s->n_sft;
+    return t;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// accumulation-kernel dispatch
+// ---------------------------------------------------------------------------------------------------------------------
+template <typename K>
+int launch_stage1(bsh_ctx *ctx, K kernel, const Stage1Params &p, int tpb, int grid, int smem)
+{
+    CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    kernel<<<grid, tpb, smem, ctx->stream>>>(p);
+    count_launch(ctx);
+    CK(cudaGetLastError());
+    return BSH_OK;
+}
+
+#define UNW_CASE(NW_, HP_, R_, CL_)                                                                                   \
+    if (pd.NW == NW_ && pd.HP == HP_ && pd.R == R_ && pd.clamp == CL_)                                                \
+        return launch_stage1(ctx, stage1_unweighted_kernel<NW_, HP_, R_, CL_>, p, pd.tpb, grid,                       \
+                             StageLayout<R_, false>(pd.n_entries).total());
+
+int dispatch_unweighted(bsh_ctx *ctx, const Pending &pd, const Stage1Params &p, int grid)
+{
+    UNW_CASE(2, 6, 2, false) UNW_CASE(2, 6, 2, true) UNW_CASE(3, 6, 2, false) UNW_CASE(3, 6, 2, true)
+    UNW_CASE(2, 8, 2, false) UNW_CASE(2, 8, 2, true) UNW_CASE(3, 8, 2, false) UNW_CASE(3, 8, 2, true)
+    UNW_CASE(2, 11, 2, false) UNW_CASE(2, 11, 2, true) UNW_CASE(3, 11, 2, false) UNW_CASE(3, 11, 2, true)
+    UNW_CASE(2, 6, 1, false) UNW_CASE(3, 6, 1, false) UNW_CASE(2, 8, 1, false) UNW_CASE(3, 8, 1, false)
+    UNW_CASE(2, 6, 1, true) UNW_CASE(3, 6, 1, true) UNW_CASE(2, 8, 1, true) UNW_CASE(3, 8, 1, true)
+    UNW_CASE(2, 11, 1, false) UNW_CASE(3, 11, 1, false) UNW_CASE(2, 11, 1, true) UNW_CASE(3, 11, 1, true)
+    return fail(ctx, BSH_EINVAL, "no unweighted kernel for NW=%d HP=%d R=%d clamp=%d", pd.NW, pd.HP, pd.R, (int)pd.clamp);
+}
+
+#define W_CASE(NW_, CL_)                                                                               \
+    if (pd.NW == NW_ && pd.clamp == CL_)                                                               \
+        return launch_stage1(ctx, stage1_weighted_kernel<NW_, CL_>, p, pd.tpb, grid,                   \
+                             StageLayout<1, true>(pd.n_entries).total());
+
+int dispatch_weighted(bsh_ctx *ctx, const Pending &pd, const Stage1Params &p, int grid)
+{
+    W_CASE(2, false) W_CASE(2, true) W_CASE(3, false) W_CASE(3, true)
+    return fail(ctx, BSH_EINVAL, "no weighted kernel for NW=%d", pd.NW);
+}
+
+// one accumulation pass over all f0 tiles with the current threshold shift
+int run_pass(bsh_ctx *ctx)
+{
+    Pending &pd = ctx->pend;
+    const TableCache &c = ctx->cache[pd.cache_slot];
+    const bool weighted = (pd.mode & BSH_WEIGHTED) != 0;
+    CK(cudaMemsetAsync(ctx->cand_count.p, 0, sizeof(unsigned int), ctx->stream));
+    threshold_kernel<<<1, 1, 0, ctx->stream>>>((const double *)ctx->stats.p, pd.frac, pd.shift_sigma, pd.emit_all ? 1 : 0,
+                                               (Threshold *)ctx->thr.p);
+    count_launch(ctx);
+    CK(cudaEventRecord(ctx->ev[2], ctx->stream));
+    if (pd.mode & BSH_NAIVE) {
+        bsh_sfts s = {};
+        s.n_sft = pd.n_sft; s.k_slab0 = pd.k_slab0; s.n_bins = pd.n_bins;
+        bsh_grid g = {};
+        g.n_pix = pd.n_pix; g.n_ap = pd.n_ap; g.n_P = pd.n_P; g.n_tasc = pd.n_tasc; g.n_f0 = pd.n_f0; g.k_band0 = pd.k_band0;
+        const TrackTables t = make_track_tables(c, &s, &g, (const double *)ctx->dtab.p, pd.R);
+        const uint64_t blocks = (pd.n_templates + 255) / 256;
+        if (blocks > 0x7FFFFFFFull) return fail(ctx, BSH_EINVAL, "naive kernel: too many templates");
+        stage1_naive_kernel<<<(unsigned)blocks, 256, 0, ctx->stream>>>(
+            t, pd.d_peak, pd.words_per_row, pd.d_w, weighted ? 1 : 0, pd.n_templates, (const Threshold *)ctx->thr.p,
+            (RawCand *)ctx->cand.p, (unsigned int *)ctx->cand_count.p, kCandCap, pd.d_counts_full);
+        count_launch(ctx);
+        CK(cudaGetLastError());
+        ctx->st.grid_blocks = (int)blocks;
+        ctx->st.threads_per_block = 256;
+    } else {
+        const int tile_bins = 32 * pd.NW;
+        for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
+            Stage1Params p;
+            p.wtab = (const uint4 *)ctx->wtab.p;
+            p.cs = (const double2 *)c.d_cs.p;
+            p.dtab = (const double *)ctx->dtab.p;
+            p.w_pad = (const float *)ctx->w_pad.p;
+            p.A = (const double *)c.d_A.p;
+            p.casa = (const double2 *)c.d_casa.p;
+            p.n_pad = pd.n_pad; p.n_entries = pd.n_entries; p.n_chunks = pd.n_pad / kChunk;
+            p.n_pix = pd.n_pix; p.n_ap = pd.n_ap; p.n_P = pd.n_P; p.n_tasc = pd.n_tasc; p.n_f0 = pd.n_f0;
+            p.j0 = j0; p.n_fj = std::min(tile_bins, pd.n_f0 - j0);
+            p.n_groups = pd.n_groups; p.n_aq = pd.n_ap * pd.n_tasc; p.n_aq_tiles = pd.n_aq_tiles;
+            p.u0 = (double)(pd.k_band0 + j0);
+            p.off = (int)(pd.k_band0 - pd.k_slab0) + j0 + pd.off_table;
+            p.s_max = pd.s_max;
+            p.thr = (const Threshold *)ctx->thr.p;
+            p.cand = (RawCand *)ctx->cand.p;
+            p.cand_count = (unsigned int *)ctx->cand_count.p;
+            p.cand_cap = kCandCap;
+            p.counts_full = pd.d_counts_full;
+            const int64_t grid = (int64_t)pd.n_groups * pd.n_P * pd.n_aq_tiles;
+            if (grid > 0x7FFFFFFFll) return fail(ctx, BSH_EINVAL, "grid too large");
+            ctx->st.grid_blocks = (int)grid;
+            ctx->st.threads_per_block = pd.tpb;
+            TRY(weighted ? dispatch_weighted(ctx, pd, p, (int)grid) : dispatch_unweighted(ctx, pd, p, (int)grid));
+        }
+    }
+    CK(cudaEventRecord(ctx->ev[3], ctx->stream));
+    pd.passes += 1;
+    return BSH_OK;
+}
+
+// sort the first n candidates of ctx->cand (buffer has room for the power-of-two padding)
+int sort_candidates(bsh_ctx *ctx, RawCand *buf, unsigned int n)
+{
+    if (n <= 1) return BSH_OK;
+    unsigned int n2 = 1;
+    while (n2 < n) n2 <<= 1;
+    if (n2 > n) {
+        pad_candidates_kernel<<<(n2 - n + 255) / 256, 256, 0, ctx->stream>>>(buf, n, n2);
+        count_launch(ctx);
+    }
+    const unsigned int tiles = (n2 + kSortTile - 1) / kSortTile;
+    const unsigned int k_local = std::min<unsigned int>(n2, kSortTile);
+    bitonic_tile_kernel<<<tiles, 1024, 0, ctx->stream>>>(buf, n2, 2u, k_local);
+    count_launch(ctx);
+    for (unsigned int k = kSortTile * 2; k <= n2; k <<= 1) {
+        for (unsigned int j = k >> 1; j >= (unsigned)kSortTile; j >>= 1) {
+            bitonic_global_kernel<<<(n2 / 2 + 255) / 256, 256, 0, ctx->stream>>>(buf, n2, k, j);
+            count_launch(ctx);
+        }
+        bitonic_tile_kernel<<<tiles, 1024, 0, ctx->stream>>>(buf, n2, k, k);
+        count_launch(ctx);
+    }
+    CK(cudaGetLastError());
+    return BSH_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================================
+// C ABI
+// =====================================================================================================================
+extern "C" {
+
+int bsh_version(void) { return 100; }
+
+int bsh_create(bsh_ctx **out, int device, void *cuda_stream)
+{
+    if (!out) return BSH_EINVAL;
+    *out = nullptr;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1 || device < 0 || device >= n_dev) return BSH_ECUDA;
+    bsh_ctx *ctx = new (std::nothrow) bsh_ctx();
+    if (!ctx) return BSH_ENOMEM;
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    if (cudaSetDevice(device) != cudaSuccess) { delete ctx; return BSH_ECUDA; }
+    for (auto &e : ctx->ev)
+        if (cudaEventCreate(&e) != cudaSuccess) { delete ctx; return BSH_ECUDA; }
+    if (cudaMallocHost((void **)&ctx->pinned_count, 64) != cudaSuccess) { delete ctx; return BSH_ENOMEM; }
+    *out = ctx;
+    return BSH_OK;
+}
+
+int bsh_destroy(bsh_ctx *ctx)
+{
+    if (!ctx) return BSH_EINVAL;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    DevBuf *bufs[] = {&ctx->wtab, &ctx->w_pad, &ctx->stats, &ctx->thr, &ctx->dtab, &ctx->nvec, &ctx->cand, &ctx->cand_count,
+                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top};
+    for (DevBuf *b : bufs)
+        if (b->p) cudaFree(b->p);
+    for (auto &c : ctx->cache) {
+        DevBuf *cb[] = {&c.d_v, &c.d_cs, &c.d_casa, &c.d_A};
+        for (DevBuf *b : cb)
+            if (b->p) cudaFree(b->p);
+    }
+    for (auto &e : ctx->ev)
+        if (e) cudaEventDestroy(e);
+    if (ctx->pinned_count) cudaFreeHost(ctx->pinned_count);
+    delete ctx;
+    return BSH_OK;
+}
+
+const char *bsh_last_error(const bsh_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int bsh_get_stats(bsh_ctx *ctx, bsh_stats *out)
+{
+    if (!ctx || !out) return BSH_EINVAL;
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaStreamSynchronize(ctx->stream));
+    float ms = 0.f;
+    if (ctx->have_pk && cudaEventElapsedTime(&ms, ctx->ev[8], ctx->ev[9]) == cudaSuccess) ctx->st.peakgram_ms = ms;
+    if (ctx->have_setup && cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]) == cudaSuccess) ctx->st.stage1_setup_ms = ms;
+    if (ctx->have_kernel && cudaEventElapsedTime(&ms, ctx->ev[2], ctx->ev[3]) == cudaSuccess)
+        ctx->st.stage1_kernel_ms = ms + ctx->kernel_ms_extra;
+    if (ctx->have_select && cudaEventElapsedTime(&ms, ctx->ev[4], ctx->ev[5]) == cudaSuccess) ctx->st.stage1_select_ms = ms;
+    if (ctx->have_s2 && cudaEventElapsedTime(&ms, ctx->ev[6], ctx->ev[7]) == cudaSuccess) ctx->st.stage2_ms = ms;
+    *out = ctx->st;
+    return BSH_OK;
+}
+
+int bsh_build_peakgram(bsh_ctx *ctx, const float *d_rho, int32_t n_sft, int32_t n_bins, int64_t rho_row_stride,
+                       float rho_th, uint32_t *d_peak, int32_t words_per_row)
+{
+    if (!ctx) return BSH_EINVAL;
+    if (!d_rho || !d_peak || n_sft < 1 || n_bins < 1 || rho_row_stride < n_bins)
+        return fail(ctx, BSH_EINVAL, "bsh_build_peakgram: bad arguments");
+    if ((int64_t)words_per_row * 32 < n_bins) return fail(ctx, BSH_ESMALL, "words_per_row * 32 < n_bins");
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaEventRecord(ctx->ev[8], ctx->stream));
+    const bool vec4 = (rho_row_stride % 4 == 0) && ((uintptr_t)d_rho % 16 == 0);
+    if (vec4) {
+        const int segs = (words_per_row + 3) / 4;
+        const int64_t warps = (int64_t)n_sft * segs;
+        peakgram_vec4_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, ctx->stream>>>(d_rho, n_sft, n_bins, rho_row_stride,
+                                                                                    rho_th, d_peak, words_per_row);
+    } else {
+        const int64_t warps = (int64_t)n_sft * words_per_row;
+        peakgram_scalar_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, ctx->stream>>>(d_rho, n_sft, n_bins, rho_row_stride,
+                                                                                      rho_th, d_peak, words_per_row);
+    }
+    count_launch(ctx);
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(ctx->ev[9], ctx->stream));
+    ctx->have_pk = true;
+    return BSH_OK;
+}
+
+int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_row, const bsh_sfts *sfts,
+                      const bsh_grid *grid, int32_t mode, int32_t topk, void *d_counts_full)
+{
+    if (!ctx) return BSH_EINVAL;
+    TRY(validate(ctx, sfts, grid));
+    if (!d_peak || topk < 1) return fail(ctx, BSH_EINVAL, "bsh_stage1: null peakgram or topk < 1");
+    if ((int64_t)words_per_row * 32 < sfts->n_bins) return fail(ctx, BSH_ESMALL, "words_per_row * 32 < n_bins");
+    if ((mode & BSH_WEIGHTED) && !sfts->d_w) return fail(ctx, BSH_EINVAL, "BSH_WEIGHTED needs sfts->d_w");
+    if (mode & ~(BSH_WEIGHTED | BSH_NAIVE)) return fail(ctx, BSH_EINVAL, "unknown mode bits");
+    CK(cudaSetDevice(ctx->device));
+    ctx->pend.active = false;
+
+    Pending pd;
+    pd.mode = mode; pd.topk = topk; pd.d_counts_full = d_counts_full; pd.d_peak = d_peak;
+    pd.words_per_row = words_per_row; pd.d_w = sfts->d_w;
+    pd.n_sft = sfts->n_sft; pd.n_bins = sfts->n_bins; pd.n_pix = grid->n_pix; pd.n_ap = grid->n_ap; pd.n_P = grid->n_P;
+    pd.n_tasc = grid->n_tasc; pd.n_f0 = grid->n_f0; pd.k_band0 = grid->k_band0; pd.k_slab0 = sfts->k_slab0;
+    pd.n_templates = (uint64_t)grid->n_pix * grid->n_ap * grid->n_P * grid->n_tasc * (uint64_t)grid->n_f0;
+    const bool weighted = (mode & BSH_WEIGHTED) != 0;
+
+    TRY(get_tables(ctx, sfts, grid, &pd.cache_slot));
+    const TableCache &c = ctx->cache[pd.cache_slot];
+    pd.n_pad = c.n_pad;
+
+    // kernel shape
+    pd.NW = grid->n_f0 <= 64 ? 2 : 3;
+    pd.R = weighted ? 1 : 2;
+    if (const char *e = getenv("BSH_PIXELS_PER_THREAD")) {
+        const int r = atoi(e);
+        if (!weighted && (r == 1 || r == 2)) pd.R = r;
+    }
+    pd.HP = sfts->n_sft < (1 << 11) ? 6 : (sfts->n_sft < (1 << 13) ? 8 : 11);
+    if (sfts->n_sft >= (1 << 16)) return fail(ctx, BSH_EINVAL, "n_sft >= 65536 not supported");
+    const TableGeometry tg = table_geometry(sfts->n_sft, sfts->h_v_over_c, grid->n_P, grid->h_P, grid->n_ap, grid->h_ap,
+                                            grid->k_band0, sfts->k_slab0, grid->n_f0, sfts->n_bins, pd.NW,
+                                            getenv("BSH_FORCE_CLAMP") != nullptr);
+    pd.clamp = tg.clamp; pd.off_table = tg.off_table; pd.s_max = tg.s_max; pd.n_entries = tg.n_entries;
+    const int n_aq = grid->n_ap * grid->n_tasc;
+    pd.tpb = pick_threads_per_block(n_aq);
+    pd.n_aq_tiles = (n_aq + pd.tpb - 1) / pd.tpb;
+    pd.n_groups = (grid->n_pix + pd.R - 1) / pd.R;
+    pd.emit_all = pd.n_templates <= kCandCap;
+    pd.frac = (double)std::max<int64_t>(8ll * topk, 4096) / (double)pd.n_templates;
+    if (pd.frac >= 0.25) pd.frac = 0.25;
+    pd.shift_sigma = 0.0;
+    pd.passes = 0;
+
+    // device scratch
+    TRY(ensure(ctx, ctx->wtab, (size_t)pd.n_pad * pd.n_entries * 16));
+    TRY(ensure(ctx, ctx->w_pad, (size_t)pd.n_pad * 4));
+    TRY(ensure(ctx, ctx->stats, 16));
+    TRY(ensure(ctx, ctx->thr, sizeof(Threshold)));
+    TRY(ensure(ctx, ctx->cand, (size_t)kCandCap * sizeof(RawCand)));
+    TRY(ensure(ctx, ctx->cand_count, 16));
+
+    CK(cudaEventRecord(ctx->ev[0], ctx->stream));
+    CK(cudaMemsetAsync(ctx->stats.p, 0, 16, ctx->stream));
+    prep_table_kernel<<<(pd.n_pad + 255) / 256, 256, 0, ctx->stream>>>(
+        d_peak, words_per_row, sfts->n_sft, pd.n_pad, sfts->n_bins, pd.n_entries, pd.off_table / 32,
+        weighted ? sfts->d_w : nullptr, (uint4 *)ctx->wtab.p, (float *)ctx->w_pad.p, (double *)ctx->stats.p);
+    count_launch(ctx);
+    CK(cudaGetLastError());
+    TRY(build_dtable(ctx, grid, c, pd.R, ctx->nvec, ctx->dtab));
+    CK(cudaEventRecord(ctx->ev[1], ctx->stream));
+    ctx->have_setup = true;
+
+    ctx->pend = pd;
+    ctx->kernel_ms_extra = 0.f;
+    TRY(run_pass(ctx));
+    ctx->have_kernel = true;
+    CK(cudaMemcpyAsync(ctx->pinned_count, ctx->cand_count.p, sizeof(unsigned int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->pinned_count + 4, ctx->thr.p, sizeof(Threshold), cudaMemcpyDeviceToHost, ctx->stream));
+    ctx->pend.active = true;
+
+    ctx->st.n_templates = (int64_t)pd.n_templates;
+    ctx->st.n_accumulations = (int64_t)pd.n_templates * sfts->n_sft;
+    ctx->st.kernel_variant = pd.NW * 100 + pd.R * 10 + (pd.clamp ? 1 : 0);
+    return BSH_OK;
+}
+
+int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
+{
+    if (!ctx) return BSH_EINVAL;
+    if (!ctx->pend.active) return fail(ctx, BSH_ESTATE, "bsh_stage1_collect without a pending bsh_stage1_launch");
+    if (!d_top || !h_n_top) return fail(ctx, BSH_EINVAL, "null d_top / h_n_top");
+    CK(cudaSetDevice(ctx->device));
+    Pending &pd = ctx->pend;
+    const bool weighted = (pd.mode & BSH_WEIGHTED) != 0;
+    const uint64_t want = std::min<uint64_t>((uint64_t)pd.topk, pd.n_templates);
+    unsigned int n_cand = 0;
+    for (;;) {
+        CK(cudaStreamSynchronize(ctx->stream));
+        n_cand = ctx->pinned_count[0];
+        const bool too_few = n_cand < want, too_many = n_cand > kCandCap;
+        if (!too_few && !too_many) break;
+        if (pd.passes >= kMaxPasses) return fail(ctx, BSH_ECUDA, "candidate selection did not converge (%u candidates)", n_cand);
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, ctx->ev[2], ctx->ev[3]) == cudaSuccess) ctx->kernel_ms_extra += ms;
+        if (too_few) {
+            pd.shift_sigma -= 0.75;
+            if (pd.passes >= 6) { pd.emit_all = true; }
+        } else {
+            pd.emit_all = false;
+            pd.shift_sigma += 0.5;
+        }
+        TRY(run_pass(ctx));
+        CK(cudaMemcpyAsync(ctx->pinned_count, ctx->cand_count.p, sizeof(unsigned int), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaMemcpyAsync(ctx->pinned_count + 4, ctx->thr.p, sizeof(Threshold), cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    Threshold thr;
+    memcpy(&thr, ctx->pinned_count + 4, sizeof thr);
+    ctx->st.n_candidates = n_cand;
+    ctx->st.threshold = weighted ? (double)thr.tau_f : (double)thr.tau_i;
+    ctx->st.n_passes = pd.passes;
+
+    CK(cudaEventRecord(ctx->ev[4], ctx->stream));
+    TRY(sort_candidates(ctx, (RawCand *)ctx->cand.p, n_cand));
+    const int n_keep = (int)want;
+    finalize_top_kernel<<<(pd.topk + 255) / 256, 256, 0, ctx->stream>>>((const RawCand *)ctx->cand.p, n_keep, pd.topk,
+                                                                      weighted ? 1 : 0, d_top);
+    count_launch(ctx);
+    {
+        const TableCache &c = ctx->cache[pd.cache_slot];
+        bsh_sfts s = {};
+        s.n_sft = pd.n_sft; s.k_slab0 = pd.k_slab0; s.n_bins = pd.n_bins;
+        bsh_grid g = {};
+        g.n_pix = pd.n_pix; g.n_ap = pd.n_ap; g.n_P = pd.n_P; g.n_tasc = pd.n_tasc; g.n_f0 = pd.n_f0; g.k_band0 = pd.k_band0;
+        const TrackTables t = make_track_tables(c, &s, &g, (const double *)ctx->dtab.p, pd.R);
+        rescore_kernel<<<(n_keep * 32 + 255) / 256, 256, 0, ctx->stream>>>(t, pd.d_peak, pd.words_per_row, pd.d_w,
+                                                                          weighted ? 1 : 0, d_top, n_keep);
+        count_launch(ctx);
+    }
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(ctx->ev[5], ctx->stream));
+    ctx->have_select = true;
+    *h_n_top = n_keep;
+    pd.active = false;
+    return BSH_OK;
+}
+
+int bsh_stage1_hough(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_row, const bsh_sfts *sfts,
+                     const bsh_grid *grid, int32_t mode, int32_t topk, bsh_cand *d_top, int32_t *h_n_top,
+                     void *d_counts_full)
+{
+    if (!ctx) return BSH_EINVAL;
+    if (!d_top || !h_n_top) return fail(ctx, BSH_EINVAL, "null d_top / h_n_top");
+    TRY(bsh_stage1_launch(ctx, d_peak, words_per_row, sfts, grid, mode, topk, d_counts_full));
+    TRY(bsh_stage1_collect(ctx, d_top, h_n_top));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return BSH_OK;
+}
+
+int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, const bsh_sfts *sfts,
+                     const bsh_grid *grid, bsh_cand *d_cands, int32_t n_cands, int32_t sort_by_power)
+{
+    if (!ctx) return BSH_EINVAL;
+    TRY(validate(ctx, sfts, grid));
+    if (!d_rho || !d_cands || n_cands < 0 || rho_row_stride < sfts->n_bins)
+        return fail(ctx, BSH_EINVAL, "bsh_stage2_power: bad arguments");
+    if (n_cands == 0) return BSH_OK;
+    CK(cudaSetDevice(ctx->device));
+    int slot = 0;
+    TRY(get_tables(ctx, sfts, grid, &slot));
+    const TableCache &c = ctx->cache[slot];
+    CK(cudaEventRecord(ctx->ev[6], ctx->stream));
+    TRY(build_dtable(ctx, grid, c, 1, ctx->nvec2, ctx->dtab2));
+    const TrackTables t = make_track_tables(c, sfts, grid, (const double *)ctx->dtab2.p, 1);
+    stage2_kernel<<<(unsigned)(((int64_t)n_cands * 32 + 255) / 256), 256, 0, ctx->stream>>>(t, d_rho, rho_row_stride,
+                                                                                          sfts->d_w, d_cands, n_cands);
+    count_launch(ctx);
+    CK(cudaGetLastError());
+    if (sort_by_power && n_cands > 1) {
+        unsigned int n2 = 1;
+        while (n2 < (unsigned)n_cands) n2 <<= 1;
+        TRY(ensure(ctx, ctx->keys, (size_t)n2 * sizeof(RawCand)));
+        TRY(ensure(ctx, ctx->tmp_cands, (size_t)n_cands * sizeof(bsh_cand)));
+        pack_power_keys_kernel<<<(n_cands + 255) / 256, 256, 0, ctx->stream>>>(d_cands, n_cands, (RawCand *)ctx->keys.p);
+        count_launch(ctx);
+        TRY(sort_candidates(ctx, (RawCand *)ctx->keys.p, (unsigned)n_cands));
+        CK(cudaMemcpyAsync(ctx->tmp_cands.p, d_cands, (size_t)n_cands * sizeof(bsh_cand), cudaMemcpyDeviceToDevice,
+                           ctx->stream));
+        permute_cands_kernel<<<(n_cands + 255) / 256, 256, 0, ctx->stream>>>((const bsh_cand *)ctx->tmp_cands.p,
+                                                                            (const RawCand *)ctx->keys.p, n_cands, d_cands);
+        count_launch(ctx);
+        CK(cudaGetLastError());
+    }
+    CK(cudaEventRecord(ctx->ev[7], ctx->stream));
+    ctx->have_s2 = true;
+    return BSH_OK;
+}
+
+int bsh_search_patch_host(bsh_ctx *ctx, const float *h_rho, const float *h_w, float rho_th, const bsh_sfts *sfts,
+                          const bsh_grid *grid, int32_t mode, int32_t topk, bsh_cand *h_top, int32_t *h_n_top)
+{
+    if (!ctx) return BSH_EINVAL;
+    TRY(validate(ctx, sfts, grid));
+    if (!h_rho || !h_top || !h_n_top || topk < 1) return fail(ctx, BSH_EINVAL, "bsh_search_patch_host: bad arguments");
+    if ((mode & BSH_WEIGHTED) && !h_w) return fail(ctx, BSH_EINVAL, "BSH_WEIGHTED needs h_w");
+    CK(cudaSetDevice(ctx->device));
+    const int N = sfts->n_sft, K = sfts->n_bins, W = (K + 31) / 32;
+    TRY(ensure(ctx, ctx->h_rho, sizeof(float) * (size_t)N * K));
+    TRY(ensure(ctx, ctx->h_w, sizeof(float) * (size_t)N));
+    TRY(ensure(ctx, ctx->h_peak, sizeof(uint32_t) * (size_t)N * W));
+    TRY(ensure(ctx, ctx->h_top, sizeof(bsh_cand) * (size_t)topk));
+    CK(cudaMemcpyAsync(ctx->h_rho.p, h_rho, sizeof(float) * (size_t)N * K, cudaMemcpyHostToDevice, ctx->stream));
+    if (h_w) CK(cudaMemcpyAsync(ctx->h_w.p, h_w, sizeof(float) * (size_t)N, cudaMemcpyHostToDevice, ctx->stream));
+    bsh_sfts s = *sfts;
+    s.d_w = h_w ? (const float *)ctx->h_w.p : nullptr;
+    TRY(bsh_build_peakgram(ctx, (const float *)ctx->h_rho.p, N, K, K, rho_th, (uint32_t *)ctx->h_peak.p, W));
+    TRY(bsh_stage1_launch(ctx, (const uint32_t *)ctx->h_peak.p, W, &s, grid, mode, topk, nullptr));
+    TRY(bsh_stage1_collect(ctx, (bsh_cand *)ctx->h_top.p, h_n_top));
+    TRY(bsh_stage2_power(ctx, (const float *)ctx->h_rho.p, K, &s, grid, (bsh_cand *)ctx->h_top.p, *h_n_top, 1));
+    CK(cudaMemcpyAsync(h_top, ctx->h_top.p, sizeof(bsh_cand) * (size_t)topk, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return BSH_OK;
+}
+
+uint64_t bsh_template_index(const bsh_grid *g, int32_t pix, int32_t ia, int32_t ip, int32_t it, int32_t j)
+{
+    return ((((uint64_t)pix * g->n_ap + ia) * g->n_P + ip) * g->n_tasc + it) * (uint64_t)g->n_f0 + j;
+}
+
+void bsh_template_decode(const bsh_grid *g, uint64_t idx, int32_t *pix, int32_t *ia, int32_t *ip, int32_t *it, int32_t *j)
+{
+    const int32_t jj = (int32_t)(idx % (uint64_t)g->n_f0);   idx /= (uint64_t)g->n_f0;
+    const int32_t tt = (int32_t)(idx % (uint64_t)g->n_tasc); idx /= (uint64_t)g->n_tasc;
+    const int32_t pp = (int32_t)(idx % (uint64_t)g->n_P);    idx /= (uint64_t)g->n_P;
+    const int32_t aa = (int32_t)(idx % (uint64_t)g->n_ap);   idx /= (uint64_t)g->n_ap;
+    if (pix) *pix = (int32_t)idx;
+    if (ia) *ia = aa;
+    if (ip) *ip = pp;
+    if (it) *it = tt;
+    if (j) *j = jj;
+}
+
+}  // extern "C"

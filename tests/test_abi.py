@@ -1,0 +1,76 @@
+"""CPU-side checks of the boundary: libbsh.so builds for sm_100a, loads, and exports every symbol include/bsh.h
+declares; pure-host entry points behave; and nothing computes without a GPU (no CPU fallback)."""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    import paper_1904_04873_b200 as b
+    lib = b.library()
+    header = open(os.path.join(ROOT, "include", "bsh.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(bsh_[a-z0-9_]+)\s*\(", header))
+    assert {"bsh_build_peakgram", "bsh_stage1_hough", "bsh_stage2_power"} <= declared
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert lib.bsh_version() >= 100
+    assert declared == set(b.binding.EXPORTS)
+
+
+def test_library_is_built_for_sm_100a_with_tma_and_fp64_no_fma():
+    import paper_1904_04873_b200 as b
+    path = b.build.build_library()
+    out = subprocess.run(["cuobjdump", "-lelf", path], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    sass = subprocess.run(["cuobjdump", "-sass", path], capture_output=True, text=True).stdout
+    kernels = sass.split("Function : ")
+    acc = [k for k in kernels if k.startswith("_ZN3bsh24stage1_unweighted_kernel") or k.startswith("_ZN3bsh22stage1_weighted_kernel")]
+    assert acc
+    for k in acc:
+        assert "UBLKCP" in k, "accumulation kernels stage their chunks with TMA bulk copies"
+        assert "DFMA" not in k, "track arithmetic must not contract to FMA (DESIGN.md R-5)"
+        assert "DMUL" in k and "DADD" in k and "LOP3" in k
+
+
+def test_template_index_roundtrip_and_order():
+    import paper_1904_04873_b200 as b
+    wl = synth.config2()
+    rng = np.random.default_rng(0)
+    for _ in range(50):
+        pix, ia, ip, it, j = (int(rng.integers(n)) for n in (64, 20, 30, 40, 90))
+        idx = b.template_index(wl, pix, ia, ip, it, j)
+        assert idx == ((((pix * 20 + ia) * 30 + ip) * 40 + it) * 90 + j)
+        assert b.template_decode(wl, idx) == (pix, ia, ip, it, j)
+    assert b.CAND_DTYPE.itemsize == 24
+
+
+def test_no_cpu_fallback():
+    import torch
+    import paper_1904_04873_b200 as b
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(b.BshError):
+        b.Context(0)
+    ctx = C.c_void_p()
+    assert b.library().bsh_create(C.byref(ctx), 0, None) < 0 and not ctx.value
+
+
+def test_product_path_does_not_import_the_oracle():
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_1904_04873_b200")):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".hpp", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle|bsh_oracle|#include\s+\"[^\"]*oracle|CDLL\([^)]*oracle", text, re.M), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(import|from)\s+paper_1904_04873_b200|#include\s+\"[^\"]*csrc|libbsh\.so", text, re.M), f

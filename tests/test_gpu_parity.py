@@ -1,0 +1,391 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle.  All tests here need a B200: -m gpu.
+
+Bars (BASELINE.json north_star): tracks, unweighted counts and unweighted toplists bit-exact against the oracle's
+CANONICAL mode; weighted counts and the stage-2 power within 1e-5 relative (FP32 accumulate vs FP64 oracle); weighted /
+power toplists identical except for ties within that tolerance at the cut.
+"""
+import dataclasses
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+import synth
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def bsh():
+    import paper_1904_04873_b200 as b
+    return b
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    return torch
+
+
+@pytest.fixture()
+def ctx(bsh):
+    c = bsh.Context(0)
+    yield c
+    c.close()
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_stage1(bsh, torch, ctx, wl, mode, topk=None, full=True, rho=None):
+    rho = wl.rho if rho is None else rho
+    d_rho = dev(torch, rho)
+    d_w = dev(torch, wl.w)
+    d_peak = ctx.build_peakgram(d_rho, 1.6)
+    weighted = bool(mode & bsh.BSH_WEIGHTED)
+    counts = None
+    if full:
+        counts = torch.full((wl.n_templates,), -7, dtype=torch.float32 if weighted else torch.int32, device="cuda")
+    d_top, n_top = ctx.stage1_hough(d_peak, wl, mode=mode, topk=topk, d_w=d_w, counts_full=counts)
+    return dict(d_rho=d_rho, d_w=d_w, d_peak=d_peak, counts=None if counts is None else counts.cpu().numpy(),
+                top=ctx.records(d_top, n_top), d_top=d_top, n_top=n_top)
+
+
+def check_unweighted_toplist(top, counts_all, k):
+    """identical toplist: (count desc, index asc) of ALL counts, by a numpy lexsort"""
+    want = np.lexsort((np.arange(counts_all.size), -counts_all.astype(np.int64)))[:k]
+    assert np.array_equal(top["index"], want.astype(np.uint64))
+    assert np.array_equal(top["count"], counts_all[want])
+
+
+def check_float_toplist(idx_got, values_ref, k, rtol=RTOL):
+    """same set as the reference top-k except for entries within rtol of the k-th value"""
+    order = np.lexsort((np.arange(values_ref.size), -values_ref))
+    want = set(order[:k].tolist())
+    got = set(int(i) for i in idx_got)
+    assert len(got) == min(k, values_ref.size)
+    cut = values_ref[order[min(k, values_ref.size) - 1]]
+    for i in want ^ got:
+        assert abs(values_ref[i] - cut) <= rtol * abs(cut), (i, values_ref[i], cut)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# peakgram
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,k", [(1, 1), (3, 31), (5, 32), (7, 33), (64, 63), (50, 172), (9, 257), (2000, 172), (8000, 252)])
+def test_peakgram_bit_exact(bsh, torch, ctx, n, k):
+    rng = np.random.default_rng(n * 1000 + k)
+    rho = rng.standard_exponential((n, k)).astype(np.float32)
+    rho[0, 0] = np.float32(1.6)
+    if k > 2:
+        rho[0, 1] = np.nextafter(np.float32(1.6), np.float32(2))
+        rho[0, 2] = np.nan
+    want = oracle.peakgram(rho)
+    got = ctx.build_peakgram(dev(torch, rho), 1.6).cpu().numpy().view(np.uint32)
+    assert np.array_equal(got, want)
+    # strided input (row stride > K) and a wider output buffer
+    wide = np.zeros((n, k + 5), np.float32)
+    wide[:, :k] = rho
+    d_wide = dev(torch, wide)
+    out = torch.full((n, want.shape[1] + 2), -1, dtype=torch.int32, device="cuda")
+    got2 = ctx.build_peakgram(d_wide[:, :k], 1.6, out=out).cpu().numpy().view(np.uint32)
+    assert np.array_equal(got2[:, :want.shape[1]], want) and not got2[:, want.shape[1]:].any()
+
+
+def test_empty_and_bad_arguments_are_rejected(bsh, torch, ctx):
+    wl = synth.config1()
+    d_rho = dev(torch, wl.rho)
+    d_peak = ctx.build_peakgram(d_rho)
+    small = torch.empty((wl.n_sft, 1), dtype=torch.int32, device="cuda")
+    with pytest.raises(bsh.BshError):
+        ctx.build_peakgram(d_rho, out=small)                         # words_per_row * 32 < n_bins
+    with pytest.raises(bsh.BshError):
+        ctx.stage1_hough(d_peak, wl, mode=bsh.BSH_WEIGHTED, d_w=None)  # weighted without weights
+    with pytest.raises(bsh.BshError):
+        ctx.stage1_hough(d_peak, wl, topk=0)
+    bad = dataclasses.replace(wl, k_band0=wl.k_slab0 - 1)
+    with pytest.raises(bsh.BshError):
+        ctx.stage1_hough(d_peak, bad)
+    with pytest.raises(bsh.BshError):
+        ctx._pending = (None, 4)                                       # collect without a pending launch
+        ctx.stage1_collect()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# config 1 (both pixels): everything, element by element
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("pixel", ["ecliptic", "pole"])
+@pytest.mark.parametrize("naive", [False, True])
+def test_config1_full_parity(bsh, torch, ctx, pixel, naive):
+    wl = synth.config1(pixel=pixel)
+    pk = oracle.peakgram(wl.rho)
+    want_n, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
+    extra = bsh.BSH_NAIVE if naive else 0
+    # unweighted
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED | extra)
+    assert np.array_equal(r["d_peak"].cpu().numpy().view(np.uint32), pk)
+    assert np.array_equal(r["counts"], want_n)
+    assert r["n_top"] == 10
+    check_unweighted_toplist(r["top"], want_n, 10)
+    assert np.allclose(r["top"]["wcount"], want_w[r["top"]["index"].astype(np.int64)], rtol=RTOL, atol=0)
+    # stage 2 on that toplist
+    ctx.stage2_power(r["d_rho"], wl, r["d_top"], r["n_top"], d_w=r["d_w"], sort_by_power=True)
+    recs = ctx.records(r["d_top"], r["n_top"])
+    want_p = oracle.stage2(wl, recs["index"], wl.rho, wl.w, mode=oracle.CANONICAL)
+    assert np.allclose(recs["power"], want_p, rtol=RTOL, atol=0)
+    assert set(recs["index"].tolist()) == set(r["top"]["index"].tolist())
+    order = np.lexsort((recs["index"], -recs["power"]))
+    assert np.array_equal(order, np.arange(len(recs)))
+    assert (recs["flags"] == 3).all()
+    # weighted
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED | extra)
+    assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=0)
+    check_float_toplist(r["top"]["index"], want_w, 10)
+    assert np.array_equal(r["top"]["count"], want_n[r["top"]["index"].astype(np.int64)])
+    assert np.allclose(r["top"]["wcount"], want_w[r["top"]["index"].astype(np.int64)], rtol=RTOL, atol=0)
+
+
+def test_topk_larger_than_template_count(bsh, torch, ctx):
+    wl = synth.noise_workload(seed=3, n_sft=40, n_f0=5, margin=20, f_band_start=100.0, n_pix_side=1, ap=(10.0,),
+                              P_days=(15.0,), n_t=2, topk=64)
+    pk = oracle.peakgram(wl.rho)
+    want_n, _ = oracle.stage1(wl, pk, None)
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=64)
+    assert r["n_top"] == wl.n_templates == 10
+    check_unweighted_toplist(r["top"], want_n, 64)
+    rest = ctx.records(r["d_top"])[10:]
+    assert not rest["flags"].any() and not rest["index"].any()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# ragged sizes: several SFT chunks + tail, several f0 tiles + tail, odd pixel counts, both table variants
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_sft,n_f0,margin,f0,side", [(1, 1, 3, 50.0, 1), (33, 7, 12, 80.0, 1), (64, 90, 30, 120.0, 2),
+                                                        (200, 96, 45, 150.0, 3), (130, 97, 45, 150.0, 2),
+                                                        (70, 200, 60, 200.0, 1), (2100, 64, 50, 180.0, 1)])
+def test_ragged_sizes(bsh, torch, ctx, monkeypatch, n_sft, n_f0, margin, f0, side):
+    wl = synth.noise_workload(seed=n_sft + n_f0, n_sft=n_sft, n_f0=n_f0, margin=margin, f_band_start=f0, n_pix_side=side,
+                              ap=(10.0, 40.0), P_days=(15.0, 31.0), n_t=3, topk=7)
+    pk = oracle.peakgram(wl.rho)
+    want_n, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
+    for force_clamp in (False, True):
+        if force_clamp:
+            monkeypatch.setenv("BSH_FORCE_CLAMP", "1")
+        else:
+            monkeypatch.delenv("BSH_FORCE_CLAMP", raising=False)
+        for ppt in ("1", "2"):
+            monkeypatch.setenv("BSH_PIXELS_PER_THREAD", ppt)
+            r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
+            assert np.array_equal(r["counts"], want_n), (force_clamp, ppt)
+            check_unweighted_toplist(r["top"], want_n, 7)
+        r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED)
+        assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=1e-6)
+        check_float_toplist(r["top"]["index"], want_w, 7)
+
+
+def test_multiple_breaks_per_band_fallback(bsh, torch, ctx):
+    wl = synth.noise_workload(seed=77, n_sft=96, n_f0=90, margin=40, f_band_start=150.0, n_pix_side=1,
+                              ap=(2500.0, 6000.0), P_days=(15.0,), n_t=4)
+    pk = oracle.peakgram(wl.rho)
+    want_n, _ = oracle.stage1(wl, pk, None, mode=oracle.CANONICAL)
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
+    assert np.array_equal(r["counts"], want_n)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# config 2: a complete sub-grid element by element, then the full grid in the bench's launch configuration
+# ------------------------------------------------------------------------------------------------------------
+def test_config2_subgrid_element_by_element(bsh, torch, ctx):
+    wl = synth.config2()
+    rng = np.random.default_rng(2)
+    sub = wl.subgrid(ia=np.sort(rng.choice(20, 3, replace=False)), ip=np.sort(rng.choice(30, 4, replace=False)),
+                     it=np.sort(rng.choice(40, 3, replace=False)))
+    pk = oracle.peakgram(wl.rho)
+    want_n, want_w = oracle.stage1(sub, pk, wl.w, mode=oracle.CANONICAL)        # 64 pix x 36 b x 90 f0 x 2000 SFTs
+    r = gpu_stage1(bsh, torch, ctx, sub, bsh.BSH_UNWEIGHTED, topk=1000)
+    assert np.array_equal(r["counts"], want_n)
+    check_unweighted_toplist(r["top"], want_n, 1000)
+    r = gpu_stage1(bsh, torch, ctx, sub, bsh.BSH_WEIGHTED, topk=1000)
+    assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=0)
+    check_float_toplist(r["top"]["index"], want_w, 1000)
+
+
+def _sampled_full_size_checks(bsh, torch, ctx, wl, weighted, n_sample=3000):
+    """Full grid: (a) toplist entries re-scored one by one by the oracle; (b) a seeded sample of ALL templates re-scored by
+    the oracle against the full dump; (c) the toplist is the true top-k of the dump (torch sort, a library routine);
+    (d) stage-2 power of the toplist against the oracle."""
+    mode = bsh.BSH_WEIGHTED if weighted else bsh.BSH_UNWEIGHTED
+    r = gpu_stage1(bsh, torch, ctx, wl, mode, topk=wl.topk)
+    st = ctx.stats()
+    pk = oracle.peakgram(wl.rho)
+    top = r["top"]
+    assert r["n_top"] == wl.topk
+    n_o, w_o, _ = oracle.score(wl, top["index"], peak=pk, w=wl.w)
+    assert np.array_equal(top["count"], n_o)
+    assert np.allclose(top["wcount"], w_o, rtol=RTOL, atol=0)
+    rng = np.random.default_rng(123)
+    idx = rng.integers(0, wl.n_templates, n_sample).astype(np.uint64)
+    n_s, w_s, _ = oracle.score(wl, idx, peak=pk, w=wl.w)
+    got = r["counts"][idx.astype(np.int64)]
+    if weighted:
+        assert np.allclose(got, w_s, rtol=RTOL, atol=0)
+    else:
+        assert np.array_equal(got, n_s)
+    # (c) toplist == top-k of the dump
+    d_counts = torch.from_numpy(r["counts"]).cuda()
+    if weighted:
+        vals, order = torch.sort(d_counts, descending=True, stable=True)
+        cut = float(vals[wl.topk - 1])
+        got_set = set(int(i) for i in top["index"])
+        want_set = set(order[:wl.topk].cpu().numpy().tolist())
+        for i in got_set ^ want_set:
+            assert abs(float(r["counts"][i]) - cut) <= RTOL * cut
+        assert np.all(np.diff(top["wcount"]) <= 0)
+    else:
+        vals, order = torch.sort(d_counts, descending=True, stable=True)
+        assert np.array_equal(top["index"], order[:wl.topk].cpu().numpy().astype(np.uint64))
+        assert np.array_equal(top["count"], vals[:wl.topk].cpu().numpy())
+    # (d) stage 2
+    ctx.stage2_power(r["d_rho"], wl, r["d_top"], r["n_top"], d_w=r["d_w"], sort_by_power=True)
+    recs = ctx.records(r["d_top"], r["n_top"])
+    p_o = oracle.stage2(wl, recs["index"], wl.rho, wl.w)
+    assert np.allclose(recs["power"], p_o, rtol=RTOL, atol=0)
+    assert np.all(np.diff(recs["power"]) <= 0)
+    return r, st
+
+
+def test_config2_full_size_unweighted(bsh, torch, ctx):
+    wl = synth.config2()
+    r, st = _sampled_full_size_checks(bsh, torch, ctx, wl, weighted=False)
+    assert st["n_templates"] == 138_240_000 and st["n_accumulations"] == 276_480_000_000
+    # the tiled kernel and the one-thread-per-template diagnostic kernel agree on every one of the 1.38e8 counts
+    rn = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED | bsh.BSH_NAIVE, topk=wl.topk)
+    assert np.array_equal(rn["counts"], r["counts"])
+    assert np.array_equal(rn["top"]["index"], r["top"]["index"])
+    # noise statistics of the full dump: Binomial(2000, e^-1.6) up to the sample's peak fraction
+    p_hat = np.unpackbits(oracle.peakgram(wl.rho).view(np.uint8)).sum() / (wl.n_sft * wl.n_bins)
+    assert abs(r["counts"].mean() - wl.n_sft * p_hat) < 1.0
+    assert abs(r["counts"].std() / math.sqrt(wl.n_sft * p_hat * (1 - p_hat)) - 1) < 0.05
+
+
+def test_config2_full_size_weighted(bsh, torch, ctx):
+    _sampled_full_size_checks(bsh, torch, ctx, synth.config2(), weighted=True)
+
+
+def test_config3_full_size_weighted(bsh, torch, ctx):
+    """BASELINE.json configs[2]: 1.66e9 templates, 8000 SFTs, weighted FP32 counts."""
+    wl = synth.config3()
+    r, st = _sampled_full_size_checks(bsh, torch, ctx, wl, weighted=True, n_sample=1500)
+    assert st["n_templates"] == 1_658_880_000
+
+
+def test_config3_full_size_unweighted_toplist(bsh, torch, ctx):
+    wl = synth.config3()
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=wl.topk, full=False)
+    pk = oracle.peakgram(wl.rho)
+    n_o, w_o, _ = oracle.score(wl, r["top"]["index"], peak=pk, w=wl.w)
+    assert np.array_equal(r["top"]["count"], n_o)
+    assert np.all(np.diff(r["top"]["count"].astype(np.int64)) <= 0)
+    ties = np.diff(r["top"]["count"].astype(np.int64)) == 0
+    assert np.all(np.diff(r["top"]["index"].astype(np.int64))[ties] > 0)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# config 4: injected signals are recovered as the loudest candidate of their patch
+# ------------------------------------------------------------------------------------------------------------
+def test_config4_signal_recovery(bsh, torch, ctx):
+    c4 = synth.config4()
+    bins = []
+    for inj in c4.injections:
+        wl_p = c4.patch_workload(inj.patch, None)
+        bins.append(oracle.track(wl_p, inj.pix, inj.ia, inj.ip, inj.it, inj.j, mode=oracle.DIRECT))
+    rho = c4.deposit(bins)
+    pk = oracle.peakgram(rho)
+    for inj in c4.injections:
+        wl = c4.patch_workload(inj.patch, rho)
+        r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=1000, full=False)
+        want = oracle.encode_index(wl, inj.pix, inj.ia, inj.ip, inj.it, inj.j)
+        assert int(r["top"]["index"][0]) == want, inj.patch
+        n_o, _, _ = oracle.score(wl, r["top"]["index"], peak=pk, w=None)
+        assert np.array_equal(r["top"]["count"], n_o)
+        p_sig = 0.29568
+        assert abs(r["top"]["count"][0] - wl.n_sft * p_sig) < 5 * math.sqrt(wl.n_sft * p_sig * (1 - p_sig))
+        ctx.stage2_power(r["d_rho"], wl, r["d_top"], r["n_top"], d_w=None, sort_by_power=True)
+        recs = ctx.records(r["d_top"], r["n_top"])
+        assert int(recs["index"][0]) == want
+        p_o = oracle.stage2(wl, recs["index"][:50], rho, None)
+        assert np.allclose(recs["power"][:50], p_o, rtol=RTOL, atol=0)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# config 5: patches streamed on two CUDA streams (two contexts), shared peakgram
+# ------------------------------------------------------------------------------------------------------------
+def test_config5_two_streams(bsh, torch):
+    c5 = synth.config5()
+    patches = [0, 100, 255, 17]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ctxs = [bsh.Context(0, stream=s) for s in streams]
+    d_rho = dev(torch, c5.base.rho)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(streams[0]):
+        d_peak = ctxs[0].build_peakgram(d_rho)
+    torch.cuda.synchronize()
+    pk = oracle.peakgram(c5.base.rho)
+    assert np.array_equal(d_peak.cpu().numpy().view(np.uint32), pk)
+    results, wls, keep = {}, {}, {}
+    pending = [None, None]
+    for n, ip in enumerate(patches + [None, None]):
+        s = n % 2
+        if pending[s] is not None:                              # collect the patch launched two steps ago on this stream
+            jp = pending[s]
+            with torch.cuda.stream(streams[s]):
+                d_top, n_top = ctxs[s].stage1_collect()
+                ctxs[s].stage2_power(d_rho, wls[jp], d_top, n_top, d_w=keep[jp], sort_by_power=True)
+            results[jp] = (d_top, n_top)
+            pending[s] = None
+        if ip is not None:
+            wls[ip] = c5.patch_workload(ip)
+            with torch.cuda.stream(streams[s]):
+                keep[ip] = dev(torch, wls[ip].w)
+                ctxs[s].stage1_launch(d_peak, wls[ip], mode=bsh.BSH_UNWEIGHTED, topk=1000, d_w=keep[ip])
+            pending[s] = ip
+    torch.cuda.synchronize()
+    for ip in patches:
+        d_top, n_top = results[ip]
+        recs = ctxs[0].records(d_top, n_top)
+        assert n_top == 1000
+        n_o, w_o, p_o = oracle.score(wls[ip], recs["index"], peak=pk, rho=c5.base.rho, w=wls[ip].w)
+        assert np.array_equal(recs["count"], n_o)
+        assert np.allclose(recs["wcount"], w_o, rtol=RTOL, atol=0)
+        assert np.allclose(recs["power"], p_o, rtol=RTOL, atol=0)
+        assert np.all(np.diff(recs["power"]) <= 0)
+    # same patch on one stream gives the same toplist
+    with torch.cuda.stream(streams[0]):
+        d_top, n_top = ctxs[0].stage1_hough(d_peak, wls[100], topk=1000, d_w=keep[100])
+        ctxs[0].stage2_power(d_rho, wls[100], d_top, n_top, d_w=keep[100], sort_by_power=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(ctxs[0].records(d_top, n_top), ctxs[0].records(results[100][0], 1000))
+    for c in ctxs:
+        c.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# the host-buffer end-to-end call
+# ------------------------------------------------------------------------------------------------------------
+def test_search_patch_host_end_to_end(bsh, torch, ctx):
+    wl = synth.config1(pixel="pole")
+    recs, n_top = ctx.search_patch_host(wl.rho, wl.w, wl, mode=bsh.BSH_UNWEIGHTED, topk=10)
+    pk = oracle.peakgram(wl.rho)
+    want_n, want_w = oracle.stage1(wl, pk, wl.w)
+    want_idx = oracle.toplist(want_n.astype(np.float64), 10)
+    assert n_top == 10 and set(recs["index"].tolist()) == set(want_idx.tolist())
+    p_o = oracle.stage2(wl, recs["index"], wl.rho, wl.w)
+    assert np.allclose(recs["power"], p_o, rtol=RTOL, atol=0)
+    assert np.array_equal(recs["count"], want_n[recs["index"].astype(np.int64)])
+    assert np.all(np.diff(recs["power"]) <= 0)
+    st = ctx.stats()
+    assert st["launches"] > 0 and st["n_templates"] == 1620
