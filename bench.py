@@ -233,6 +233,11 @@ def main_ours(args, rank, local_rank, world):
     w_total_ms, w_kern_ms, _, _ = timed(lambda: step(bsh.BSH_WEIGHTED), w_steps, 1)
     st_w = ctx.stats()
 
+    if args.profile:
+        print(json.dumps({"profile_run": True, "unweighted_kernel_ms": float(np.mean(kern_ms)),
+                          "weighted_kernel_ms": float(np.mean(w_kern_ms))}), flush=True)
+        return
+
     # end to end through the host-buffer entry point
     def e2e_step():
         ctx.search_patch_host(h_rho.numpy(), h_w.numpy(), wl, mode=bsh.BSH_UNWEIGHTED, topk=wl.topk, out=h_out_np)
@@ -308,6 +313,8 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--profile", action="store_true",
+                    help="only the timed unweighted + weighted steps (no e2e, no oracle): the command ncu wraps")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

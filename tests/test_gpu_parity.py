@@ -268,7 +268,8 @@ def test_config2_full_size_unweighted(bsh, torch, ctx):
     assert np.array_equal(rn["top"]["index"], r["top"]["index"])
     # noise statistics of the full dump: Binomial(2000, e^-1.6) up to the sample's peak fraction
     p_hat = np.unpackbits(oracle.peakgram(wl.rho).view(np.uint8)).sum() / (wl.n_sft * wl.n_bins)
-    assert abs(r["counts"].mean() - wl.n_sft * p_hat) < 1.0
+    # (p_hat has a sampling error of sqrt(p(1-p)/(N K)) = 7e-4, i.e. 1.4 counts: allow 4 sigma)
+    assert abs(r["counts"].mean() - wl.n_sft * p_hat) < 6.0
     assert abs(r["counts"].std() / math.sqrt(wl.n_sft * p_hat * (1 - p_hat)) - 1) < 0.05
 
 
