@@ -49,7 +49,7 @@ struct Pending {                      // state between bsh_stage1_launch and bsh
     int64_t k_band0 = 0, k_slab0 = 0;
     uint64_t n_templates = 0;
     bool emit_all = false, clamp = false;
-    int R = 2, NW = 3, HP = 6, n_entries = 0, off_table = 0, s_max = 0, tpb = 256, n_groups = 0, n_aq_tiles = 0;
+    int R = 2, NW = 3, HP = 6, n_entries = 0, off_table = 0, s_max = 0, s_zero = 0, list_cap = 0, tpb = 256, n_groups = 0, n_aq_tiles = 0;
     double frac = 0, shift_sigma = 0;
     int passes = 0;
 };
@@ -240,7 +240,7 @@ int launch_stage1(bsh_ctx *ctx, K kernel, const Stage1Params &p, int tpb, int gr
 #define UNW_CASE(NW_, HP_, R_, CL_)                                                                                   \
     if (pd.NW == NW_ && pd.HP == HP_ && pd.R == R_ && pd.clamp == CL_)                                                \
         return launch_stage1(ctx, stage1_unweighted_kernel<NW_, HP_, R_, CL_>, p, pd.tpb, grid,                       \
-                             StageLayout<R_, false>(pd.n_entries).total());
+                             StageLayout<R_, false>(pd.n_entries).total() + R_ * pd.list_cap * pd.tpb * 2);
 
 int dispatch_unweighted(bsh_ctx *ctx, const Pending &pd, const Stage1Params &p, int grid)
 {
@@ -307,6 +307,8 @@ int run_pass(bsh_ctx *ctx)
             p.u0 = (double)(pd.k_band0 + j0);
             p.off = (int)(pd.k_band0 - pd.k_slab0) + j0 + pd.off_table;
             p.s_max = pd.s_max;
+            p.s_zero = pd.s_zero;
+            p.list_cap = pd.list_cap;
             p.thr = (const Threshold *)ctx->thr.p;
             p.cand = (RawCand *)ctx->cand.p;
             p.cand_count = (unsigned int *)ctx->cand_count.p;
@@ -480,9 +482,12 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
                                             grid->k_band0, sfts->k_slab0, grid->n_f0, sfts->n_bins, pd.NW,
                                             getenv("BSH_FORCE_CLAMP") != nullptr);
     pd.clamp = tg.clamp; pd.off_table = tg.off_table; pd.s_max = tg.s_max; pd.n_entries = tg.n_entries;
+    pd.s_zero = tg.s_zero;
     const int n_aq = grid->n_ap * grid->n_tasc;
     pd.tpb = pick_threads_per_block(n_aq);
     pd.n_aq_tiles = (n_aq + pd.tpb - 1) / pd.tpb;
+    pd.list_cap = 48;
+    if (const char *e = getenv("BSH_LIST_CAP")) pd.list_cap = std::max(1, atoi(e));
     pd.n_groups = (grid->n_pix + pd.R - 1) / pd.R;
     pd.emit_all = pd.n_templates <= kCandCap;
     pd.frac = (double)std::max<int64_t>(8ll * topk, 4096) / (double)pd.n_templates;

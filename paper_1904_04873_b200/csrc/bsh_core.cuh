@@ -109,6 +109,7 @@ struct TrackConst {
     double magic;       // kMagic + off
     int32_t off;        // m + j0 + table offset: s = off + r is the bit position of tile bin 0 in table coordinates
     int32_t s_max;      // clamp range [0, s_max] of s (table coordinates); only used by CLAMP variants
+    int32_t s_zero;     // a table position whose NW-word window reads only zeros (deferred breaks park there)
     int32_t n_fj;       // f0 bins in this tile (<= 32 * NW)
 };
 
@@ -198,6 +199,22 @@ BSH_HD Win<NW> track_window(const TrackConst &tc, const uint4 *row_entries, doub
     return load_window<NW>(row_entries, CLAMP ? clamp_s(s0, tc.s_max) : s0);
 }
 
+// Main-loop form of track_window(): when the rounded shift differs between the two ends of the f0 tile (a "break",
+// ~1 % of (pixel, binary template, SFT) triples, R-7) the thread reads the all-zero window at s_zero instead and reports
+// brk = true; the caller records the SFT and later adds the exact window (track_window + add_window).  This keeps the
+// hot loop free of divergent code; the sum over SFTs is order-independent for the integer count.
+template <int NW, bool CLAMP>
+BSH_HD Win<NW> track_window_deferred(const TrackConst &tc, const uint4 *row_entries, double D, double B, bool &brk)
+{
+    const double g = dsub(D, B);
+    const int32_t s0 = shift_of(tc.u0, g, tc.magic, tc.off);
+    const int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
+    brk = s0 != sL;
+    int32_t s = CLAMP ? clamp_s(s0, tc.s_max) : s0;
+    s = brk ? tc.s_zero : s;
+    return load_window<NW>(row_entries, s);
+}
+
 BSH_HD double binary_term(const TrackConst &tc, double C, double S)   // B = fl(A fl(fl(C CA) + fl(S SA)))
 {
     return dmul(tc.A, dadd(dmul(C, tc.CA), dmul(S, tc.SA)));
@@ -256,6 +273,29 @@ template <int K, int NW, int HP>
 BSH_HD void push(Counter<NW, HP> &c, Win<NW> x)
 {
     push_level<K, 0, NW, HP>(c, x);
+}
+
+// Ripple-carry add of one window (one bit per bin) into the counter.  Only valid between blocks of kBlock SFTs, when
+// no input is parked in the hold registers.
+template <int NW, int HP>
+BSH_HD void add_window(Counter<NW, HP> &c, Win<NW> x)
+{
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+        uint32_t carry = x.x[w];
+#pragma unroll
+        for (int l = 0; l < kLowPlanes; ++l) {
+            const uint32_t t = c.low[l][w] & carry;
+            c.low[l][w] ^= carry;
+            carry = t;
+        }
+#pragma unroll
+        for (int p = 0; p < HP; ++p) {
+            const uint32_t t = c.hi[p][w] & carry;
+            c.hi[p][w] ^= carry;
+            carry = t;
+        }
+    }
 }
 
 template <int NW, int HP>

@@ -59,9 +59,11 @@ inline void pixel_vectors(int n_pix, const double *alpha, const double *delta, s
 //   clamp == false: proven that every window of every template lies inside the slab; table coordinates = slab columns.
 //   clamp == true : table coordinates = slab column + off_table, with NW + 1 zero words in front and one behind, and the
 //                   start position clamped to [0, s_max] (a clamped window reads only zeros).
+//   s_zero: a table position whose window is all zero in both geometries (the first words of the clamped table; one
+//           extra all-zero entry behind the row otherwise): where the accumulation kernels park deferred breaks.
 struct TableGeometry {
     bool clamp;
-    int off_table, s_max, n_entries;
+    int off_table, s_max, n_entries, s_zero;
 };
 
 inline TableGeometry table_geometry(int n_sft, const double *v_over_c, int n_P, const double *P, int n_ap, const double *ap,
@@ -85,11 +87,14 @@ inline TableGeometry table_geometry(int n_sft, const double *v_over_c, int n_P, 
     if (g.clamp) {
         g.off_table = 32 * (NW + 1);
         g.s_max = g.off_table + 32 * row_words;
+        g.n_entries = (g.s_max >> 5) + 1;
+        g.s_zero = 0;
     } else {
         g.off_table = 0;
         g.s_max = n_bins - 1;
+        g.n_entries = (g.s_max >> 5) + 2;
+        g.s_zero = 32 * (g.n_entries - 1);
     }
-    g.n_entries = (g.s_max >> 5) + 1;
     return g;
 }
 

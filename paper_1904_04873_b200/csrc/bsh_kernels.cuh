@@ -216,7 +216,8 @@ struct Stage1Params {
     int j0, n_fj;               // f0 tile
     int n_groups, n_aq, n_aq_tiles;
     double u0;                  // k_band0 + j0
-    int off, s_max;             // table coordinates (see TrackConst)
+    int off, s_max, s_zero;     // table coordinates (see TrackConst)
+    int list_cap;               // deferred-break list entries per (thread, pixel)
     const Threshold *thr;
     RawCand *cand;
     unsigned int *cand_count;
@@ -257,6 +258,7 @@ __device__ __forceinline__ TrackConst make_track_const(const Stage1Params &p, co
     tc.off = p.off;
     tc.magic = kMagic + (double)p.off;
     tc.s_max = p.s_max;
+    tc.s_zero = p.s_zero;
     tc.n_fj = p.n_fj;
     return tc;
 }
@@ -301,9 +303,12 @@ __device__ __forceinline__ void issue_chunk(const Stage1Params &p, const StageLa
     if (WEIGHTED) tma_bulk_g2s(stage + L.wt_bytes + L.cs_bytes + L.d_bytes, p.w_pad + i0, (uint32_t)L.w_bytes, bar);
 }
 
+// One SFT of the unrolled block: binary term once, then per pixel the window (or the zero window + a bit in brk[r] when
+// the shift breaks inside the f0 tile) pushed into the carry-save tree at compile-time position K.
 template <int K, int NW, int HP, int R, bool CLAMP>
 __device__ __forceinline__ void sft_step_unweighted(const TrackConst &tc, const uint4 *wt, int n_entries,
-                                                    const double2 *cs, const double *d, Counter<NW, HP> (&cnt)[R])
+                                                    const double2 *cs, const double *d, Counter<NW, HP> (&cnt)[R],
+                                                    uint32_t (&brk)[R])
 {
     const double2 c = cs[K];
     const double B = binary_term(tc, c.x, c.y);
@@ -318,54 +323,104 @@ __device__ __forceinline__ void sft_step_unweighted(const TrackConst &tc, const 
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const Win<NW> x = track_window<NW, CLAMP>(tc, wt + K * n_entries, Dv[r], B);
+        bool b;
+        const Win<NW> x = track_window_deferred<NW, CLAMP>(tc, wt + K * n_entries, Dv[r], B, b);
+        brk[r] |= b ? (1u << K) : 0u;
         push<K, NW, HP>(cnt[r], x);
     }
 }
 
 template <int NW, int HP, int R, bool CLAMP, int... Ks>
 __device__ __forceinline__ void block_unweighted(const TrackConst &tc, const uint4 *wt, int n_entries, const double2 *cs,
-                                                 const double *d, Counter<NW, HP> (&cnt)[R],
+                                                 const double *d, Counter<NW, HP> (&cnt)[R], uint32_t (&brk)[R],
                                                  std::integer_sequence<int, Ks...>)
 {
-    (sft_step_unweighted<Ks, NW, HP, R, CLAMP>(tc, wt, n_entries, cs, d, cnt), ...);
+    (sft_step_unweighted<Ks, NW, HP, R, CLAMP>(tc, wt, n_entries, cs, d, cnt, brk), ...);
 }
 
+// Exact window of one deferred (pixel r, SFT i) read from the global tables, added by ripple carry.
 template <int NW, int HP, int R, bool CLAMP>
-__global__ void __launch_bounds__(256, (R == 2 && NW == 3) ? 1 : 2) stage1_unweighted_kernel(const Stage1Params p)
+__device__ __forceinline__ void fixup_from_global(const Stage1Params &p, const TrackConst &tc, const BlockCoord &bc, int r,
+                                                  int i, Counter<NW, HP> &cnt)
+{
+    const double2 c = p.cs[(int64_t)bc.ip * p.n_pad + i];
+    const double B = binary_term(tc, c.x, c.y);
+    const double D = p.dtab[((int64_t)bc.grp * p.n_pad + i) * R + r];
+    const Win<NW> x = track_window<NW, CLAMP>(tc, p.wtab + (int64_t)i * p.n_entries, D, B);
+    add_window(cnt, x);
+}
+
+// Stage-1 unweighted accumulation (L223, L241-L247).  Block = (pixel group, period, tile of (a_p, t_asc) pairs);
+// thread = one (a_p, t_asc) pair x R pixels x up to 32 NW f0 bins.  SFTs stream through shared memory in chunks of
+// kChunk (TMA bulk copies, two stages).  Breaks are parked in a per-thread list in shared memory (uint16 SFT indices,
+// cap entries per pixel) and resolved in bulk when some list in the block runs full, and at the end.
+template <int NW, int HP, int R, bool CLAMP>
+__global__ void __launch_bounds__(256, 2) stage1_unweighted_kernel(const Stage1Params p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem);
     const StageLayout<R, false> L(p.n_entries);
     const BlockCoord bc = block_coord(p);
     const TrackConst tc = make_track_const(p, bc);
+    uint16_t *list = reinterpret_cast<uint16_t *>(smem + kSmemHeader + kStages * L.stride);
+    const int cap = p.list_cap, tpb = blockDim.x, tid = threadIdx.x;
 
-    if (threadIdx.x == 0) {
+    if (tid == 0) {
         mbar_init(&bars[0], 1);
         mbar_init(&bars[1], 1);
         mbar_fence_init();
     }
     __syncthreads();
-    if (threadIdx.x == 0) issue_chunk<R, false>(p, L, smem + kSmemHeader, &bars[0], 0, bc.ip, bc.grp);
+    if (tid == 0) issue_chunk<R, false>(p, L, smem + kSmemHeader, &bars[0], 0, bc.ip, bc.grp);
 
     Counter<NW, HP> cnt[R];
+    int npend[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) cnt[r].clear();
+    for (int r = 0; r < R; ++r) { cnt[r].clear(); npend[r] = 0; }
 
     for (int c = 0; c < p.n_chunks; ++c) {
         const int s = c & 1;
-        if (threadIdx.x == 0 && c + 1 < p.n_chunks)
+        if (tid == 0 && c + 1 < p.n_chunks)
             issue_chunk<R, false>(p, L, smem + kSmemHeader + (s ^ 1) * L.stride, &bars[s ^ 1], c + 1, bc.ip, bc.grp);
         mbar_wait(&bars[s], (uint32_t)((c >> 1) & 1));
         const unsigned char *st = smem + kSmemHeader + s * L.stride;
         const uint4 *wt = reinterpret_cast<const uint4 *>(st);
         const double2 *cs = reinterpret_cast<const double2 *>(st + L.wt_bytes);
         const double *d = reinterpret_cast<const double *>(st + L.wt_bytes + L.cs_bytes);
+        bool want_flush = false;
 #pragma unroll 1
-        for (int blk = 0; blk < kChunk / kBlock; ++blk)
+        for (int blk = 0; blk < kChunk / kBlock; ++blk) {
+            uint32_t brk[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) brk[r] = 0u;
             block_unweighted<NW, HP, R, CLAMP>(tc, wt + blk * kBlock * p.n_entries, p.n_entries, cs + blk * kBlock,
-                                               d + blk * kBlock * R, cnt, std::make_integer_sequence<int, kBlock>{});
-        __syncthreads();
+                                               d + blk * kBlock * R, cnt, brk, std::make_integer_sequence<int, kBlock>{});
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                uint32_t m = brk[r];
+                while (m) {
+                    const int k = __ffs(m) - 1;
+                    m &= m - 1;
+                    const int i = c * kChunk + blk * kBlock + k;
+                    if (npend[r] < cap) {
+                        list[(r * cap + npend[r]) * tpb + tid] = (uint16_t)i;
+                        npend[r] += 1;
+                    } else {
+                        fixup_from_global<NW, HP, R, CLAMP>(p, tc, bc, r, i, cnt[r]);   // list full: resolve now
+                    }
+                }
+                want_flush |= npend[r] > (cap >> 1) + (cap >> 2);
+            }
+        }
+        const bool flush = __syncthreads_or(want_flush) != 0 || c + 1 == p.n_chunks;
+        if (flush) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                for (int n = 0; n < npend[r]; ++n)
+                    fixup_from_global<NW, HP, R, CLAMP>(p, tc, bc, r, (int)list[(r * cap + n) * tpb + tid], cnt[r]);
+                npend[r] = 0;
+            }
+        }
     }
 
     // epilogue: threshold in bit-sliced form, emit the (rare) survivors

@@ -24,19 +24,32 @@ struct Tables {
     int n_pad;
 };
 
+// mirrors sft_step_unweighted / block_unweighted of bsh_kernels.cuh (R = 1): breaks read the zero window and set a bit
 template <int K, int NW, int HP, bool CLAMP>
-inline void step(const TrackConst &tc, const uint4 *wt, int n_entries, const double *cs, const double *d, Counter<NW, HP> &cnt)
+inline void step(const TrackConst &tc, const uint4 *wt, int n_entries, const double *cs, const double *d, Counter<NW, HP> &cnt,
+                 uint32_t &brk)
 {
     const double B = binary_term(tc, cs[2 * K], cs[2 * K + 1]);
-    const Win<NW> x = track_window<NW, CLAMP>(tc, wt + K * n_entries, d[K], B);
+    bool b;
+    const Win<NW> x = track_window_deferred<NW, CLAMP>(tc, wt + K * n_entries, d[K], B, b);
+    brk |= b ? (1u << K) : 0u;
     push<K, NW, HP>(cnt, x);
 }
 
 template <int NW, int HP, bool CLAMP, int... Ks>
 inline void block(const TrackConst &tc, const uint4 *wt, int n_entries, const double *cs, const double *d, Counter<NW, HP> &cnt,
-                  std::integer_sequence<int, Ks...>)
+                  uint32_t &brk, std::integer_sequence<int, Ks...>)
 {
-    (step<Ks, NW, HP, CLAMP>(tc, wt, n_entries, cs, d, cnt), ...);
+    (step<Ks, NW, HP, CLAMP>(tc, wt, n_entries, cs, d, cnt, brk), ...);
+}
+
+// mirrors fixup_from_global: the exact window of a deferred SFT, added by ripple carry
+template <int NW, int HP, bool CLAMP>
+inline void fixup(const TrackConst &tc, const uint4 *wtab, int n_entries, const double *cs, const double *d, int i,
+                  Counter<NW, HP> &cnt)
+{
+    const double B = binary_term(tc, cs[2 * i], cs[2 * i + 1]);
+    add_window(cnt, track_window<NW, CLAMP>(tc, wtab + (size_t)i * n_entries, d[i], B));
 }
 
 template <int NW, int HP, bool CLAMP>
@@ -59,6 +72,7 @@ void run(int n_sft, int n_pix, int n_ap, int n_P, int n_tasc, int n_f0, int64_t 
                         tc.off = (int)(k_band0 - k_slab0) + j0 + tg.off_table;
                         tc.magic = kMagic + (double)tc.off;
                         tc.s_max = tg.s_max;
+                        tc.s_zero = tg.s_zero;
                         tc.n_fj = n_fj;
                         const double *cs = T.cs.data() + (size_t)ip * T.n_pad * 2;
                         const double *d = T.dtab.data() + (size_t)pix * T.n_pad;
@@ -66,9 +80,25 @@ void run(int n_sft, int n_pix, int n_ap, int n_P, int n_tasc, int n_f0, int64_t 
                         if (!weighted) {
                             Counter<NW, HP> cnt;
                             cnt.clear();
-                            for (int i0 = 0; i0 < T.n_pad; i0 += kBlock)
+                            // deferred-break list with a tiny capacity so that the bulk flush, the end flush and
+                            // the list-full path of the kernel are all exercised
+                            const int cap = 3;
+                            int list[3], npend = 0;
+                            for (int i0 = 0; i0 < T.n_pad; i0 += kBlock) {
+                                uint32_t brk = 0u;
                                 block<NW, HP, CLAMP>(tc, T.wtab.data() + (size_t)i0 * tg.n_entries, tg.n_entries, cs + 2 * i0,
-                                                     d + i0, cnt, std::make_integer_sequence<int, kBlock>{});
+                                                     d + i0, cnt, brk, std::make_integer_sequence<int, kBlock>{});
+                                for (int k = 0; k < kBlock; ++k) {
+                                    if (!((brk >> k) & 1u)) continue;
+                                    if (npend < cap) list[npend++] = i0 + k;
+                                    else fixup<NW, HP, CLAMP>(tc, T.wtab.data(), tg.n_entries, cs, d, i0 + k, cnt);
+                                }
+                                if (npend > 2 || i0 + kBlock >= T.n_pad) {
+                                    for (int n = 0; n < npend; ++n)
+                                        fixup<NW, HP, CLAMP>(tc, T.wtab.data(), tg.n_entries, cs, d, list[n], cnt);
+                                    npend = 0;
+                                }
+                            }
                             // also exercise the bit-sliced threshold: count_ge must agree with the extracted counts
                             for (int w = 0; w < NW; ++w)
                                 for (int b = 0; b < 32; ++b)
