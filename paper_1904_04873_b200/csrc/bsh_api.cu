@@ -485,6 +485,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     pd.s_zero = tg.s_zero;
     const int n_aq = grid->n_ap * grid->n_tasc;
     pd.tpb = pick_threads_per_block(n_aq);
+    if (const char *e = getenv("BSH_TPB")) pd.tpb = std::max(32, std::min(256, atoi(e) / 32 * 32));
     pd.n_aq_tiles = (n_aq + pd.tpb - 1) / pd.tpb;
     pd.list_cap = 48;
     if (const char *e = getenv("BSH_LIST_CAP")) pd.list_cap = std::max(1, atoi(e));
