@@ -15,6 +15,7 @@
 #include "../../include/bsh.h"
 #include "bsh_host.hpp"
 #include "bsh_kernels.cuh"
+#include "bsh_pos.cuh"
 
 using namespace bsh;
 
@@ -52,6 +53,9 @@ struct Pending {                      // state between bsh_stage1_launch and bsh
     int R = 2, NW = 3, HP = 6, n_entries = 0, off_table = 0, s_max = 0, s_zero = 0, list_cap = 0, tpb = 256, n_groups = 0, n_aq_tiles = 0;
     double frac = 0, shift_sigma = 0;
     int passes = 0;
+    // position-table kernels (bsh_pos.cuh)
+    bool use_pos = false;
+    int pos_off = 0, pos_s_max = 0, pos_s_zero = 0, n_pos = 0, n_stages = 0, n_oct = 0, pos_groups = 0, pos_smem = 0;
 };
 
 }  // namespace
@@ -62,7 +66,7 @@ struct bsh_ctx {
     std::string err;
     TableCache cache[2];
     uint64_t stamp = 0;
-    DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2;
+    DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2, ptab, dpos;
     DevBuf h_rho, h_w, h_peak, h_top;                  // device staging of bsh_search_patch_host
     unsigned int *pinned_count = nullptr;
     cudaEvent_t ev[10] = {};
@@ -227,8 +231,8 @@ TrackTables make_track_tables(const TableCache &c, const bsh_sfts *s, const bsh_
 // ---------------------------------------------------------------------------------------------------------------------
 // accumulation-kernel dispatch
 // ---------------------------------------------------------------------------------------------------------------------
-template <typename K>
-int launch_stage1(bsh_ctx *ctx, K kernel, const Stage1Params &p, int tpb, int grid, int smem)
+template <typename K, typename P>
+int launch_stage1(bsh_ctx *ctx, K kernel, const P &p, int tpb, int grid, int smem)
 {
     CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     kernel<<<grid, tpb, smem, ctx->stream>>>(p);
@@ -264,6 +268,30 @@ int dispatch_weighted(bsh_ctx *ctx, const Pending &pd, const Stage1Params &p, in
     return fail(ctx, BSH_EINVAL, "no weighted kernel for NW=%d", pd.NW);
 }
 
+#define UNW_POS_CASE(NW_, HP_, CL_)                                                                   \
+    if (pd.NW == NW_ && pd.HP == HP_ && pd.clamp == CL_)                                              \
+        return launch_stage1(ctx, stage1_unweighted_pos_kernel<NW_, HP_, CL_>, p, 32 * kWarpsUnweighted, grid, pd.pos_smem);
+
+int dispatch_unweighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p, int grid)
+{
+    UNW_POS_CASE(2, 6, false) UNW_POS_CASE(2, 6, true) UNW_POS_CASE(3, 6, false) UNW_POS_CASE(3, 6, true)
+    UNW_POS_CASE(2, 8, false) UNW_POS_CASE(2, 8, true) UNW_POS_CASE(3, 8, false) UNW_POS_CASE(3, 8, true)
+    UNW_POS_CASE(2, 11, false) UNW_POS_CASE(2, 11, true) UNW_POS_CASE(3, 11, false) UNW_POS_CASE(3, 11, true)
+    return fail(ctx, BSH_EINVAL, "no unweighted position kernel for NW=%d HP=%d clamp=%d", pd.NW, pd.HP, (int)pd.clamp);
+}
+
+#define W_POS_CASE(NW_, NB_, CL_)                                                                     \
+    if (pd.NW == NW_ && nb == NB_ && pd.clamp == CL_)                                                 \
+        return launch_stage1(ctx, stage1_weighted_pos_kernel<NW_, NB_, CL_>, p, 32 * kWarpsWeighted, grid, pd.pos_smem);
+
+int dispatch_weighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p, int grid)
+{
+    const int nb = pd.NW == 2 ? 64 : (p.n_fj <= 90 ? 90 : 96);
+    W_POS_CASE(2, 64, false) W_POS_CASE(2, 64, true) W_POS_CASE(3, 90, false) W_POS_CASE(3, 90, true)
+    W_POS_CASE(3, 96, false) W_POS_CASE(3, 96, true)
+    return fail(ctx, BSH_EINVAL, "no weighted position kernel for NW=%d", pd.NW);
+}
+
 // one accumulation pass over all f0 tiles with the current threshold shift
 int run_pass(bsh_ctx *ctx)
 {
@@ -290,6 +318,35 @@ int run_pass(bsh_ctx *ctx)
         CK(cudaGetLastError());
         ctx->st.grid_blocks = (int)blocks;
         ctx->st.threads_per_block = 256;
+    } else if (pd.use_pos) {
+        const int tile_bins = 32 * pd.NW;
+        for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
+            PosParams p;
+            p.ptab = (const uint4 *)ctx->ptab.p;
+            p.cs = (const double2 *)c.d_cs.p;
+            p.dpos = (const double *)ctx->dpos.p;
+            p.w_pad = (const float *)ctx->w_pad.p;
+            p.A = (const double *)c.d_A.p;
+            p.casa = (const double2 *)c.d_casa.p;
+            p.n_pad = pd.n_pad; p.n_pos = pd.n_pos; p.n_chunks = pd.n_pad / kStageSfts; p.n_stages = pd.n_stages;
+            p.n_pix = pd.n_pix; p.n_ap = pd.n_ap; p.n_P = pd.n_P; p.n_tasc = pd.n_tasc; p.n_f0 = pd.n_f0;
+            p.j0 = j0; p.n_fj = std::min(tile_bins, pd.n_f0 - j0);
+            p.n_groups = pd.pos_groups; p.n_oct = pd.n_oct; p.n_aq = pd.n_ap * pd.n_tasc; p.n_aq_tiles = (p.n_aq + 31) / 32;
+            p.u0 = (double)(pd.k_band0 + j0);
+            p.off = (int)(pd.k_band0 - pd.k_slab0) + j0 + pd.pos_off;
+            p.s_max = pd.pos_s_max;
+            p.s_zero = pd.pos_s_zero;
+            p.thr = (const Threshold *)ctx->thr.p;
+            p.cand = (RawCand *)ctx->cand.p;
+            p.cand_count = (unsigned int *)ctx->cand_count.p;
+            p.cand_cap = kCandCap;
+            p.counts_full = pd.d_counts_full;
+            const int64_t grid = (int64_t)pd.n_oct * pd.n_P * p.n_aq_tiles;
+            if (grid > 0x7FFFFFFFll) return fail(ctx, BSH_EINVAL, "grid too large");
+            ctx->st.grid_blocks = (int)grid;
+            ctx->st.threads_per_block = 32 * (weighted ? kWarpsWeighted : kWarpsUnweighted);
+            TRY(weighted ? dispatch_weighted_pos(ctx, pd, p, (int)grid) : dispatch_unweighted_pos(ctx, pd, p, (int)grid));
+        }
     } else {
         const int tile_bins = 32 * pd.NW;
         for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
@@ -385,7 +442,7 @@ int bsh_destroy(bsh_ctx *ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf *bufs[] = {&ctx->wtab, &ctx->w_pad, &ctx->stats, &ctx->thr, &ctx->dtab, &ctx->nvec, &ctx->cand, &ctx->cand_count,
-                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top};
+                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto &c : ctx->cache) {
@@ -490,6 +547,22 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     pd.list_cap = 48;
     if (const char *e = getenv("BSH_LIST_CAP")) pd.list_cap = std::max(1, atoi(e));
     pd.n_groups = (grid->n_pix + pd.R - 1) / pd.R;
+    {   // position-table kernels when 2+ stages of the table fit in shared memory (else the funnel-shift kernels)
+        const PosGeometry pg = pos_geometry(tg, sfts->n_bins, grid->n_f0, pd.NW);
+        pd.pos_off = pg.off_table; pd.pos_s_max = pg.s_max; pd.pos_s_zero = pg.s_zero; pd.n_pos = pg.n_pos;
+        const int wpb = weighted ? kWarpsWeighted : kWarpsUnweighted;
+        const int stride = weighted ? PosStage<kWarpsWeighted, 1, true>(pg.n_pos).stride
+                                    : PosStage<kWarpsUnweighted, 2, false>(pg.n_pos).stride;
+        const int budgets[3] = {weighted ? 74 * 1024 : 112 * 1024, 112 * 1024, 224 * 1024};   // 3 / 2 / 1 blocks per SM
+        pd.n_stages = 0;
+        for (int b = 0; b < 3 && pd.n_stages < 2; ++b) pd.n_stages = std::min(kMaxStages, (budgets[b] - kPosHeader) / stride);
+        if (const char *e = getenv("BSH_STAGES")) pd.n_stages = std::min(pd.n_stages, std::max(2, atoi(e)));
+        pd.use_pos = pd.n_stages >= 2 && getenv("BSH_LEGACY") == nullptr && !(mode & BSH_NAIVE);
+        pd.n_stages = std::min(pd.n_stages, pd.n_pad / kStageSfts);
+        pd.pos_groups = weighted ? grid->n_pix : (grid->n_pix + 1) / 2;
+        pd.n_oct = (pd.pos_groups + wpb - 1) / wpb;
+        pd.pos_smem = kPosHeader + pd.n_stages * stride;
+    }
     pd.emit_all = pd.n_templates <= kCandCap;
     pd.frac = (double)std::max<int64_t>(8ll * topk, 4096) / (double)pd.n_templates;
     if (pd.frac >= 0.25) pd.frac = 0.25;
@@ -512,6 +585,22 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     count_launch(ctx);
     CK(cudaGetLastError());
     TRY(build_dtable(ctx, grid, c, pd.R, ctx->nvec, ctx->dtab));
+    if (pd.use_pos) {
+        const int wpb = weighted ? kWarpsWeighted : kWarpsUnweighted, R = weighted ? 1 : 2;
+        TRY(ensure(ctx, ctx->ptab, (size_t)pd.n_pad * pd.n_pos * 16));
+        TRY(ensure(ctx, ctx->dpos, sizeof(double) * (size_t)pd.n_oct * pd.n_pad * wpb * R));
+        const int64_t n_ent = (int64_t)pd.n_pad * pd.n_pos;
+        build_position_table_kernel<<<(unsigned)((n_ent + 255) / 256), 256, 0, ctx->stream>>>(
+            d_peak, words_per_row, sfts->n_sft, pd.n_pad, sfts->n_bins, pd.n_pos, pd.pos_off, pd.pos_s_zero,
+            (uint4 *)ctx->ptab.p);
+        count_launch(ctx);
+        const int64_t n_d = (int64_t)pd.n_oct * pd.n_pad * wpb * R;
+        dtable_pos_kernel<<<(unsigned)((n_d + 255) / 256), 256, 0, ctx->stream>>>(
+            (const double *)c.d_v.p, (const double *)ctx->nvec.p, c.n_sft, pd.n_pad, grid->n_pix, pd.n_oct, wpb, R,
+            (double *)ctx->dpos.p);
+        count_launch(ctx);
+        CK(cudaGetLastError());
+    }
     CK(cudaEventRecord(ctx->ev[1], ctx->stream));
     ctx->have_setup = true;
 
@@ -525,7 +614,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
 
     ctx->st.n_templates = (int64_t)pd.n_templates;
     ctx->st.n_accumulations = (int64_t)pd.n_templates * sfts->n_sft;
-    ctx->st.kernel_variant = pd.NW * 100 + pd.R * 10 + (pd.clamp ? 1 : 0);
+    ctx->st.kernel_variant = (pd.use_pos ? 1000 : 0) + pd.NW * 100 + pd.R * 10 + (pd.clamp ? 1 : 0);
     return BSH_OK;
 }
 

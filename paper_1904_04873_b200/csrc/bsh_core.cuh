@@ -221,6 +221,85 @@ BSH_HD double binary_term(const TrackConst &tc, double C, double S)   // B = fl(
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
+// Pre-shifted window table ("position table"): entry p of SFT i holds the NW window words of a window STARTING at table
+// position p (x, y, z = words 0..2; w unused), so the hot loop needs no funnel shift and no entry/bit split: one 16-byte
+// load at row + p.  Position p is slab column (p - off_table) of tile bin 0; bits outside [0, K) are zero.  TrackConst
+// is used unchanged: s = off + r is the position, [0, s_max] the clamp range, s_zero an all-zero position.
+// ---------------------------------------------------------------------------------------------------------------------
+template <int NW>
+BSH_HD Win<NW> load_position(const uint4 *row_positions, int32_t s)
+{
+    const uint4 e = row_positions[s];
+    Win<NW> w;
+    w.x[0] = e.x;
+    if (NW > 1) w.x[1 % NW] = e.y;
+    if (NW > 2) w.x[2 % NW] = e.z;
+    return w;
+}
+
+// Exact window of a break (R-7) from the position table: one break -> blend of the two neighbouring positions at the
+// break bin (located on the canonical evaluation itself); several breaks -> every bin from its own position.
+template <int NW, bool CLAMP>
+BSH_HD_NOINLINE Win<NW> break_window_pos(const uint4 *row_positions, double g, double u0, double magic, int32_t off,
+                                         int32_t n_fj, int32_t s_max, int32_t s0, int32_t sL)
+{
+    Win<NW> out;
+    const int32_t d = sL - s0;
+    if (d == 1 || d == -1) {
+        int lo = 0, hi = n_fj - 1;                       // shift(lo) == s0, shift(hi) == sL
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            const int32_t sm = shift_of(dadd(u0, (double)mid), g, magic, off);
+            if (sm == s0) lo = mid; else hi = mid;
+        }
+        const Win<NW> a = load_position<NW>(row_positions, CLAMP ? clamp_s(s0, s_max) : s0);
+        const Win<NW> b = load_position<NW>(row_positions, CLAMP ? clamp_s(sL, s_max) : sL);
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+            const int rel = hi - 32 * w;                 // bins j >= hi take the second window
+            const uint32_t m = rel <= 0 ? 0xFFFFFFFFu : (rel >= 32 ? 0u : (0xFFFFFFFFu << rel));
+            out.x[w] = (a.x[w] & ~m) | (b.x[w] & m);
+        }
+        return out;
+    }
+#pragma unroll
+    for (int w = 0; w < NW; ++w) out.x[w] = 0u;
+    for (int j = 0; j < n_fj; ++j) {
+        int32_t sj = shift_of(dadd(u0, (double)j), g, magic, off);
+        sj = clamp_s(sj, s_max);                         // in the unclamped geometry this is the identity (proven range)
+        const uint4 e = row_positions[sj];
+        const uint32_t word = (j >> 5) == 0 ? e.x : ((j >> 5) == 1 ? e.y : e.z);
+        const uint32_t bit = (word >> (j & 31)) & 1u;
+#pragma unroll
+        for (int w = 0; w < NW; ++w)
+            if ((j >> 5) == w) out.x[w] |= bit << (j & 31);
+    }
+    return out;
+}
+
+template <int NW, bool CLAMP>
+BSH_HD Win<NW> track_window_pos(const TrackConst &tc, const uint4 *row_positions, double D, double B)
+{
+    const double g = dsub(D, B);
+    const int32_t s0 = shift_of(tc.u0, g, tc.magic, tc.off);
+    const int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
+    if (s0 != sL) return break_window_pos<NW, CLAMP>(row_positions, g, tc.u0, tc.magic, tc.off, tc.n_fj, tc.s_max, s0, sL);
+    return load_position<NW>(row_positions, CLAMP ? clamp_s(s0, tc.s_max) : s0);
+}
+
+// Hot-loop form: the position to read (the all-zero position on a break) and the break flag.
+template <bool CLAMP>
+BSH_HD int32_t track_position_deferred(const TrackConst &tc, double D, double B, bool &brk)
+{
+    const double g = dsub(D, B);
+    int32_t s0 = shift_of(tc.u0, g, tc.magic, tc.off);
+    int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
+    if (CLAMP) { s0 = clamp_s(s0, tc.s_max); sL = clamp_s(sL, tc.s_max); }   // equal after clamping => every bin reads 0
+    brk = s0 != sL;
+    return brk ? tc.s_zero : s0;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
 // Unweighted: bit-sliced counter.  32 lanes of a word are 32 f0 bins; plane p holds bit p of each bin's count.
 // Inputs arrive in blocks of 32 SFTs; within a block a carry-save adder tree (one full adder = 2 LOP3 per word) keeps
 // planes 0..4 and emits one weight-32 carry per block, which is rippled into the HP high planes.

@@ -98,6 +98,33 @@ inline TableGeometry table_geometry(int n_sft, const double *v_over_c, int n_P, 
     return g;
 }
 
+// Geometry of the position table (pre-shifted windows, bsh_core.cuh) derived from the window-table geometry `tg`:
+//   clamp == false: position = slab column of tile bin 0, valid range [0, K - w_min] (w_min = narrowest f0 tile);
+//                   one extra all-zero position behind it (s_zero).
+//   clamp == true : position = slab column + 32 NW, clamped to [0, K + 32 NW]; both ends are all-zero windows.
+struct PosGeometry {
+    int off_table, s_max, n_pos, s_zero;
+};
+
+inline PosGeometry pos_geometry(const TableGeometry &tg, int n_bins, int n_f0, int NW)
+{
+    PosGeometry g;
+    if (tg.clamp) {
+        g.off_table = 32 * NW;
+        g.s_max = n_bins + 32 * NW;
+        g.n_pos = g.s_max + 1;
+        g.s_zero = 0;
+    } else {
+        const int tile = 32 * NW;
+        const int w_min = n_f0 <= tile ? n_f0 : ((n_f0 % tile) ? (n_f0 % tile) : tile);
+        g.off_table = 0;
+        g.s_max = n_bins - w_min;
+        g.s_zero = g.s_max + 1;
+        g.n_pos = g.s_max + 2;
+    }
+    return g;
+}
+
 inline int pick_threads_per_block(int n_aq)
 {
     int best = 64;
