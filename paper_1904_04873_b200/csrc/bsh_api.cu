@@ -16,6 +16,7 @@
 #include "bsh_host.hpp"
 #include "bsh_kernels.cuh"
 #include "bsh_pos.cuh"
+#include "bsh_pix.cuh"
 
 using namespace bsh;
 
@@ -56,6 +57,9 @@ struct Pending {                      // state between bsh_stage1_launch and bsh
     // position-table kernels (bsh_pos.cuh)
     bool use_pos = false;
     int pos_off = 0, pos_s_max = 0, pos_s_zero = 0, n_pos = 0, n_stages = 0, n_oct = 0, pos_groups = 0, pos_smem = 0;
+    // pixel-lane kernel (bsh_pix.cuh)
+    bool use_pix = false;
+    int n_pg = 0, pix_stages = 0, pix_smem = 0;
 };
 
 }  // namespace
@@ -66,7 +70,7 @@ struct bsh_ctx {
     std::string err;
     TableCache cache[2];
     uint64_t stamp = 0;
-    DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2, ptab, dpos;
+    DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2, ptab, dpos, dpix;
     DevBuf h_rho, h_w, h_peak, h_top;                  // device staging of bsh_search_patch_host
     unsigned int *pinned_count = nullptr;
     cudaEvent_t ev[10] = {};
@@ -280,6 +284,18 @@ int dispatch_unweighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p,
     return fail(ctx, BSH_EINVAL, "no unweighted position kernel for NW=%d HP=%d clamp=%d", pd.NW, pd.HP, (int)pd.clamp);
 }
 
+#define UNW_PIX_CASE(NW_, HP_, CL_)                                                                   \
+    if (pd.NW == NW_ && pd.HP == HP_ && pd.clamp == CL_)                                              \
+        return launch_stage1(ctx, stage1_unweighted_pix_kernel<NW_, HP_, CL_>, p, 32 * kPixWarps, grid, pd.pix_smem);
+
+int dispatch_unweighted_pix(bsh_ctx *ctx, const Pending &pd, const PixParams &p, int grid)
+{
+    UNW_PIX_CASE(2, 6, false) UNW_PIX_CASE(2, 6, true) UNW_PIX_CASE(3, 6, false) UNW_PIX_CASE(3, 6, true)
+    UNW_PIX_CASE(2, 8, false) UNW_PIX_CASE(2, 8, true) UNW_PIX_CASE(3, 8, false) UNW_PIX_CASE(3, 8, true)
+    UNW_PIX_CASE(2, 11, false) UNW_PIX_CASE(2, 11, true) UNW_PIX_CASE(3, 11, false) UNW_PIX_CASE(3, 11, true)
+    return fail(ctx, BSH_EINVAL, "no unweighted pixel-lane kernel for NW=%d HP=%d clamp=%d", pd.NW, pd.HP, (int)pd.clamp);
+}
+
 #define W_POS_CASE(NW_, NB_, CL_)                                                                     \
     if (pd.NW == NW_ && nb == NB_ && pd.clamp == CL_)                                                 \
         return launch_stage1(ctx, stage1_weighted_pos_kernel<NW_, NB_, CL_>, p, 32 * kWarpsWeighted, grid, pd.pos_smem);
@@ -318,6 +334,34 @@ int run_pass(bsh_ctx *ctx)
         CK(cudaGetLastError());
         ctx->st.grid_blocks = (int)blocks;
         ctx->st.threads_per_block = 256;
+    } else if (pd.use_pix && !weighted) {
+        const int tile_bins = 32 * pd.NW;
+        for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
+            PixParams p;
+            p.ptab = (const uint4 *)ctx->ptab.p;
+            p.cs = (const double2 *)c.d_cs.p;
+            p.dpix = (const double *)ctx->dpix.p;
+            p.A = (const double *)c.d_A.p;
+            p.casa = (const double2 *)c.d_casa.p;
+            p.n_pad = pd.n_pad; p.n_pos = pd.n_pos; p.n_chunks = pd.n_pad / kStageSfts; p.n_stages = pd.pix_stages;
+            p.n_pix = pd.n_pix; p.n_ap = pd.n_ap; p.n_P = pd.n_P; p.n_tasc = pd.n_tasc; p.n_f0 = pd.n_f0;
+            p.j0 = j0; p.n_fj = std::min(tile_bins, pd.n_f0 - j0);
+            p.n_pg = pd.n_pg; p.n_aq = pd.n_ap * pd.n_tasc; p.n_aq_tiles = (p.n_aq + kPixTile - 1) / kPixTile;
+            p.u0 = (double)(pd.k_band0 + j0);
+            p.off = (int)(pd.k_band0 - pd.k_slab0) + j0 + pd.pos_off;
+            p.s_max = pd.pos_s_max;
+            p.s_zero = pd.pos_s_zero;
+            p.thr = (const Threshold *)ctx->thr.p;
+            p.cand = (RawCand *)ctx->cand.p;
+            p.cand_count = (unsigned int *)ctx->cand_count.p;
+            p.cand_cap = kCandCap;
+            p.counts_full = pd.d_counts_full;
+            const int64_t grid = (int64_t)pd.n_pg * pd.n_P * p.n_aq_tiles;
+            if (grid > 0x7FFFFFFFll) return fail(ctx, BSH_EINVAL, "grid too large");
+            ctx->st.grid_blocks = (int)grid;
+            ctx->st.threads_per_block = 32 * kPixWarps;
+            TRY(dispatch_unweighted_pix(ctx, pd, p, (int)grid));
+        }
     } else if (pd.use_pos) {
         const int tile_bins = 32 * pd.NW;
         for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
@@ -442,7 +486,7 @@ int bsh_destroy(bsh_ctx *ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf *bufs[] = {&ctx->wtab, &ctx->w_pad, &ctx->stats, &ctx->thr, &ctx->dtab, &ctx->nvec, &ctx->cand, &ctx->cand_count,
-                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top};
+                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto &c : ctx->cache) {
@@ -562,6 +606,17 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         pd.pos_groups = weighted ? grid->n_pix : (grid->n_pix + 1) / 2;
         pd.n_oct = (pd.pos_groups + wpb - 1) / wpb;
         pd.pos_smem = kPosHeader + pd.n_stages * stride;
+        // pixel-lane kernel (unweighted): pixels on the lanes pay off when most of the 32 lanes of a group are used
+        const PixStage ps(pg.n_pos);
+        pd.n_pg = (grid->n_pix + 31) / 32;
+        pd.pix_stages = 0;
+        for (int b = 1; b < 3 && pd.pix_stages < 2; ++b) pd.pix_stages = std::min(kMaxStages, (budgets[b] - kPixHeader) / ps.stride);
+        if (const char *e = getenv("BSH_STAGES")) pd.pix_stages = std::min(pd.pix_stages, std::max(2, atoi(e)));
+        const bool lanes_ok = 10 * grid->n_pix >= 6 * 32 * pd.n_pg;
+        pd.use_pix = !weighted && pd.pix_stages >= 2 && (lanes_ok || getenv("BSH_FORCE_PIX") != nullptr) &&
+                     getenv("BSH_LEGACY") == nullptr && getenv("BSH_NO_PIX") == nullptr && !(mode & BSH_NAIVE);
+        pd.pix_stages = std::max(1, std::min(pd.pix_stages, pd.n_pad / kStageSfts));
+        pd.pix_smem = kPixHeader + pd.pix_stages * ps.stride;
     }
     pd.emit_all = pd.n_templates <= kCandCap;
     pd.frac = (double)std::max<int64_t>(8ll * topk, 4096) / (double)pd.n_templates;
@@ -585,7 +640,21 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     count_launch(ctx);
     CK(cudaGetLastError());
     TRY(build_dtable(ctx, grid, c, pd.R, ctx->nvec, ctx->dtab));
-    if (pd.use_pos) {
+    if (pd.use_pix) {
+        TRY(ensure(ctx, ctx->ptab, (size_t)pd.n_pad * pd.n_pos * 16));
+        TRY(ensure(ctx, ctx->dpix, sizeof(double) * (size_t)pd.n_pg * pd.n_pad * 32));
+        const int64_t n_ent = (int64_t)pd.n_pad * pd.n_pos;
+        build_position_table_kernel<<<(unsigned)((n_ent + 255) / 256), 256, 0, ctx->stream>>>(
+            d_peak, words_per_row, sfts->n_sft, pd.n_pad, sfts->n_bins, pd.n_pos, pd.pos_off, pd.pos_s_zero,
+            (uint4 *)ctx->ptab.p);
+        count_launch(ctx);
+        const int64_t n_d = (int64_t)pd.n_pg * pd.n_pad * 32;
+        dtable_pix_kernel<<<(unsigned)((n_d + 255) / 256), 256, 0, ctx->stream>>>(
+            (const double *)c.d_v.p, (const double *)ctx->nvec.p, c.n_sft, pd.n_pad, grid->n_pix, pd.n_pg,
+            (double *)ctx->dpix.p);
+        count_launch(ctx);
+        CK(cudaGetLastError());
+    } else if (pd.use_pos) {
         const int wpb = weighted ? kWarpsWeighted : kWarpsUnweighted, R = weighted ? 1 : 2;
         TRY(ensure(ctx, ctx->ptab, (size_t)pd.n_pad * pd.n_pos * 16));
         TRY(ensure(ctx, ctx->dpos, sizeof(double) * (size_t)pd.n_oct * pd.n_pad * wpb * R));
@@ -614,7 +683,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
 
     ctx->st.n_templates = (int64_t)pd.n_templates;
     ctx->st.n_accumulations = (int64_t)pd.n_templates * sfts->n_sft;
-    ctx->st.kernel_variant = (pd.use_pos ? 1000 : 0) + pd.NW * 100 + pd.R * 10 + (pd.clamp ? 1 : 0);
+    ctx->st.kernel_variant = (pd.use_pix ? 2000 : pd.use_pos ? 1000 : 0) + pd.NW * 100 + pd.R * 10 + (pd.clamp ? 1 : 0);
     return BSH_OK;
 }
 

@@ -1,0 +1,327 @@
+// bsh_pix.cuh -- stage-1 unweighted accumulation kernel with SKY PIXELS ON THE LANES ("pixel-lane" mapping), sm_100a.
+//
+// The position-table kernel of bsh_pos.cuh puts 32 different binary templates on the lanes of a warp.  Their tracks are
+// unrelated, so the 32 16-byte window reads of one (warp, SFT) scatter over the staged table row and the kernel is bound
+// by shared-memory wavefronts (ncu: 5.2 wavefronts per LDS.128, l1tex data pipe 78 % busy).  Here a warp holds ONE
+// pair of binary templates and 32 neighbouring sky pixels:
+//   * the pixels of a patch are less than one frequency bin apart per pixel step (Eq. 34), so the 32 positions
+//     of a warp fall into a handful of consecutive table entries: same entry -> broadcast, neighbours -> different
+//     banks.  The window read costs 2 wavefronts instead of 5;
+//   * the binary term B = A (C CA + S SA) of Eq. (15) (L102) is the same for all lanes.  Each lane computes ONE of the
+//     warp's 2 x 16 values per stage and the warp shares them through shared memory, so the hot loop spends no FP64
+//     work on it (9 -> 7 FP64 operations per (pixel, template, SFT) triple);
+//   * breaks of the rounded shift inside the f0 tile (R-7) are flagged by comparing the two magic-add results as
+//     doubles (FP64 pipe, not the integer pipe) and recorded in a 32-bit mask per block of 32 SFTs.
+// Thread = 1 pixel x 2 templates x up to 32 NW f0 bins; block = 8 warps = 16 templates of one period, 32 pixels.
+//
+//   PAPER.md L102 Eq. (15) track, L223 number count, L241-L247 "loop over the binary templates"; R-5, R-7.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <utility>
+
+#include "bsh_pos.cuh"
+
+namespace bsh {
+
+constexpr int kPixWarps = 8;                         // warps per block
+constexpr int kPixTpl = 2;                           // binary templates per thread
+constexpr int kPixTile = kPixWarps * kPixTpl;        // binary templates per block
+constexpr int kPixWarpScratch = 2 * kStageSfts * kPixTpl * 8 + kPixTpl * 32;   // two B buffers + template constants
+constexpr int kPixHeader = 128 + kPixWarps * kPixWarpScratch;
+
+// D table for the pixel-lane kernel: dpix[pg][i / 2][lane][i & 1] = v_i . n_pix / c (canonical order, R-5) for pixel
+// pg * 32 + lane; padding SFTs get 0, padding lanes repeat the last real pixel (never written out).  One LDS.128 per
+// lane returns the values of two consecutive SFTs.
+__global__ void __launch_bounds__(256) dtable_pix_kernel(const double *__restrict__ v_over_c, const double *__restrict__ nvec,
+                                                         int n_sft, int n_pad, int n_pix, int n_pg,
+                                                         double *__restrict__ dpix)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t total = (int64_t)n_pg * n_pad * 32;
+    if (t >= total) return;
+    const int e = (int)(t & 1);
+    const int lane = (int)((t >> 1) & 31);
+    const int64_t q = t >> 6;
+    const int half = n_pad >> 1;
+    const int i = 2 * (int)(q % half) + e;
+    const int pg = (int)(q / half);
+    int pix = pg * 32 + lane;
+    if (pix >= n_pix) pix = n_pix - 1;
+    double D = 0.0;
+    if (i < n_sft) {
+        const double a = __dmul_rn(v_over_c[3 * i + 0], nvec[3 * pix + 0]);
+        const double b = __dmul_rn(v_over_c[3 * i + 1], nvec[3 * pix + 1]);
+        const double c = __dmul_rn(v_over_c[3 * i + 2], nvec[3 * pix + 2]);
+        D = __dadd_rn(__dadd_rn(a, b), c);
+    }
+    dpix[t] = D;
+}
+
+struct PixParams {
+    const uint4 *ptab;          // [n_pad][n_pos]
+    const double2 *cs;          // [n_P][n_pad]  (cos, sin)(Omega_p t_i)
+    const double *dpix;         // [n_pg][n_pad / 2][32][2]
+    const double *A;            // [n_ap][n_P]
+    const double2 *casa;        // [n_P][n_tasc]
+    int n_pad, n_pos, n_chunks, n_stages;
+    int n_pix, n_ap, n_P, n_tasc, n_f0;
+    int j0, n_fj;               // f0 tile
+    int n_pg, n_aq, n_aq_tiles;
+    double u0;                  // k_band0 + j0
+    int off, s_max, s_zero;     // position coordinates (TrackConst)
+    const Threshold *thr;
+    RawCand *cand;
+    unsigned int *cand_count;
+    unsigned int cand_cap;
+    void *counts_full;
+};
+
+struct PixStage {
+    int tab_bytes, cs_bytes, d_bytes, stride;
+    __device__ __host__ PixStage(int n_pos)
+    {
+        tab_bytes = kStageSfts * n_pos * 16;
+        cs_bytes = kStageSfts * 16;
+        d_bytes = kStageSfts * 32 * 8;
+        stride = tab_bytes + cs_bytes + d_bytes;
+    }
+    __device__ __host__ int total(int n_stages) const { return kPixHeader + n_stages * stride; }
+};
+
+__device__ __forceinline__ void pix_issue(const PixParams &p, const PixStage &L, unsigned char *stage, uint64_t *bar, int chunk,
+                                          int ip, int pg)
+{
+    const int64_t i0 = (int64_t)chunk * kStageSfts;
+    mbar_expect_tx(bar, (uint32_t)L.stride);
+    tma_bulk_g2s(stage, p.ptab + i0 * p.n_pos, (uint32_t)L.tab_bytes, bar);
+    tma_bulk_g2s(stage + L.tab_bytes, p.cs + (int64_t)ip * p.n_pad + i0, (uint32_t)L.cs_bytes, bar);
+    tma_bulk_g2s(stage + L.tab_bytes + L.cs_bytes, p.dpix + ((int64_t)pg * p.n_pad + i0) * 32, (uint32_t)L.d_bytes, bar);
+}
+
+// A warp is done with `stage`: the warp that releases it last refills it with chunk c + n_stages.
+__device__ __forceinline__ void pix_release(const PixParams &p, const PixStage &L, unsigned char *smem, int st, int c, int lane,
+                                            int ip, int pg)
+{
+    __syncwarp();
+    if (lane == 0) {
+        unsigned int *done = reinterpret_cast<unsigned int *>(smem + 8 * kMaxStages) + st;
+        unsigned int old;
+        asm volatile("atom.acq_rel.cta.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(done)) : "memory");
+        if ((old + 1u) % (unsigned)kPixWarps == 0u && c + p.n_stages < p.n_chunks)
+            pix_issue(p, L, smem + kPixHeader + st * L.stride, reinterpret_cast<uint64_t *>(smem) + st, c + p.n_stages, ip, pg);
+    }
+}
+
+// Per-thread constants of the hot loop (the binary-term constants live in shared memory, only the fix-ups need them).
+struct PixConst {
+    double u0, uL, magic;
+    int32_t s_max, s_zero;
+};
+
+// Position (table entry) to read for one (pixel, template, SFT) and the break flag (R-7): the all-zero position on a
+// break.  Unclamped geometry: the two magic-add results are compared as doubles (equal doubles <=> equal low words),
+// which keeps the comparison on the FP64 pipe.
+template <bool CLAMP>
+__device__ __forceinline__ int32_t pix_position(const PixConst &k, double D, double B, bool &brk)
+{
+    const double g = __dsub_rn(D, B);
+    const double m0 = __dadd_rd(__dadd_rn(__dmul_rn(k.u0, g), 0.5), k.magic);
+    const double mL = __dadd_rd(__dadd_rn(__dmul_rn(k.uL, g), 0.5), k.magic);
+    int32_t s0 = __double2loint(m0);
+    if (CLAMP) {
+        int32_t sL = __double2loint(mL);
+        s0 = clamp_s(s0, k.s_max);
+        sL = clamp_s(sL, k.s_max);                       // equal after clamping => every bin reads 0
+        brk = s0 != sL;
+    } else {
+        brk = m0 != mL;
+    }
+    return brk ? k.s_zero : s0;
+}
+
+// One SFT (slot K of the unrolled block of 32) for both templates of the thread.
+template <int K, int NW, int HP, bool CLAMP>
+__device__ __forceinline__ void pix_step(const PixConst &k, const uint4 *tab, int n_pos, const double2 *bpair,
+                                         const double2 *dpair, Counter<NW, HP> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl])
+{
+    constexpr int kk = K % kStageSfts;
+    const double2 d2 = dpair[(kk >> 1) * 32];
+    const double D = (kk & 1) ? d2.y : d2.x;
+    const double2 b2 = bpair[kk];
+    const double Bv[kPixTpl] = {b2.x, b2.y};
+#pragma unroll
+    for (int r = 0; r < kPixTpl; ++r) {
+        bool b;
+        const int32_t s = pix_position<CLAMP>(k, D, Bv[r], b);
+        brk[r] |= b ? (1u << K) : 0u;
+        push<K, NW, HP>(cnt[r], load_position<NW>(tab + kk * n_pos, s));
+    }
+}
+
+template <int K0, int NW, int HP, bool CLAMP, int... Ks>
+__device__ __forceinline__ void pix_half(const PixConst &k, const uint4 *tab, int n_pos, const double2 *bpair,
+                                         const double2 *dpair, Counter<NW, HP> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl],
+                                         std::integer_sequence<int, Ks...>)
+{
+    (pix_step<K0 + Ks, NW, HP, CLAMP>(k, tab, n_pos, bpair, dpair, cnt, brk), ...);
+}
+
+template <int NW, int HP, bool CLAMP>
+__global__ void __launch_bounds__(32 * kPixWarps, 2) stage1_unweighted_pix_kernel(const PixParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem);
+    const PixStage L(p.n_pos);
+    int b = blockIdx.x;
+    const int tile = b % p.n_aq_tiles;
+    b /= p.n_aq_tiles;
+    const int ip = b % p.n_P;
+    const int pg = b / p.n_P;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned char *wscr = smem + 128 + warp * kPixWarpScratch;
+    double *bbuf = reinterpret_cast<double *>(wscr);                               // [2 halves][16 SFTs][2 templates]
+    double *tcst = reinterpret_cast<double *>(wscr + 2 * kStageSfts * kPixTpl * 8); // [2 templates][A, CA, SA, -]
+
+    // the warp's two binary templates (a_p, t_asc pairs of period ip); a missing one repeats the last real pair
+    int ia[kPixTpl], it[kPixTpl];
+    bool act[kPixTpl];
+#pragma unroll
+    for (int r = 0; r < kPixTpl; ++r) {
+        int aq = tile * kPixTile + warp * kPixTpl + r;
+        act[r] = aq < p.n_aq;
+        if (!act[r]) aq = p.n_aq - 1;
+        ia[r] = aq / p.n_tasc;
+        it[r] = aq - ia[r] * p.n_tasc;
+    }
+    // lane l computes the binary term of template (l & 1) at SFT (l >> 1) of every stage
+    const int rd = lane & 1;
+    const double A_d = p.A[(rd ? ia[1] : ia[0]) * p.n_P + ip];
+    const double2 q_d = p.casa[ip * p.n_tasc + (rd ? it[1] : it[0])];
+    if (lane < kPixTpl) {
+        tcst[lane * 4 + 0] = A_d;
+        tcst[lane * 4 + 1] = q_d.x;
+        tcst[lane * 4 + 2] = q_d.y;
+    }
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kMaxStages; ++s) {
+            mbar_init(&full[s], 1);
+            reinterpret_cast<unsigned int *>(smem + 8 * kMaxStages)[s] = 0u;
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int n0 = p.n_stages < p.n_chunks ? p.n_stages : p.n_chunks;
+        for (int s = 0; s < n0; ++s) pix_issue(p, L, smem + kPixHeader + s * L.stride, &full[s], s, ip, pg);
+    }
+
+    PixConst kc;
+    kc.u0 = p.u0;
+    kc.uL = p.u0 + (double)(p.n_fj - 1);
+    kc.magic = kMagic + (double)p.off;
+    kc.s_max = p.s_max;
+    kc.s_zero = p.s_zero;
+
+    Counter<NW, HP> cnt[kPixTpl];
+    uint16_t list[kPixTpl][kListCap];
+    int npend[kPixTpl];
+#pragma unroll
+    for (int r = 0; r < kPixTpl; ++r) {
+        cnt[r].clear();
+        npend[r] = 0;
+    }
+
+    int st = 0;
+    uint32_t parity = 0u;
+    const int n_blocks = p.n_chunks >> 1;                // n_pad is a multiple of 32
+    for (int blk = 0; blk < n_blocks; ++blk) {
+        uint32_t brk[kPixTpl] = {0u, 0u};
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            mbar_wait(&full[st], parity);
+            const unsigned char *sp = smem + kPixHeader + st * L.stride;
+            const double2 *cs = reinterpret_cast<const double2 *>(sp + L.tab_bytes);
+            {   // binary terms of this stage: B = fl(A fl(fl(C CA) + fl(S SA)))  (R-5), one per lane
+                const double2 c = cs[lane >> 1];
+                bbuf[half * 32 + lane] = __dmul_rn(A_d, __dadd_rn(__dmul_rn(c.x, q_d.x), __dmul_rn(c.y, q_d.y)));
+                __syncwarp();
+            }
+            const double2 *bpair = reinterpret_cast<const double2 *>(bbuf + half * 32);
+            const double2 *dpair = reinterpret_cast<const double2 *>(sp + L.tab_bytes + L.cs_bytes) + lane;
+            if (half == 0)
+                pix_half<0, NW, HP, CLAMP>(kc, reinterpret_cast<const uint4 *>(sp), p.n_pos, bpair, dpair, cnt, brk,
+                                           std::make_integer_sequence<int, kStageSfts>{});
+            else
+                pix_half<kStageSfts, NW, HP, CLAMP>(kc, reinterpret_cast<const uint4 *>(sp), p.n_pos, bpair, dpair, cnt, brk,
+                                                    std::make_integer_sequence<int, kStageSfts>{});
+            pix_release(p, L, smem, st, 2 * blk + half, lane, ip, pg);
+            if (++st == p.n_stages) { st = 0; parity ^= 1u; }
+        }
+        // note the SFTs whose shift broke inside the tile; resolve the lists when one could overflow, and at the end
+        bool want = false;
+#pragma unroll
+        for (int r = 0; r < kPixTpl; ++r) {
+            uint32_t m = brk[r];
+            while (m) {
+                const int k = __ffs(m) - 1;
+                m &= m - 1;
+                list[r][npend[r]] = (uint16_t)(blk * kBlock + k);
+                npend[r] += 1;
+            }
+            want = want || npend[r] > kListCap - kBlock;
+        }
+        if (__any_sync(0xFFFFFFFFu, want) || blk + 1 == n_blocks) {
+#pragma unroll
+            for (int r = 0; r < kPixTpl; ++r) {
+                TrackConst tc;
+                tc.u0 = kc.u0; tc.uL = kc.uL; tc.magic = kc.magic; tc.off = p.off; tc.s_max = p.s_max; tc.s_zero = p.s_zero;
+                tc.n_fj = p.n_fj;
+                tc.A = tcst[r * 4 + 0]; tc.CA = tcst[r * 4 + 1]; tc.SA = tcst[r * 4 + 2];
+                for (int n = 0; n < npend[r]; ++n) {
+                    const int i = (int)list[r][n];
+                    const double2 c = p.cs[(int64_t)ip * p.n_pad + i];
+                    const double B = binary_term(tc, c.x, c.y);
+                    const double D = p.dpix[((((int64_t)pg * (p.n_pad >> 1)) + (i >> 1)) * 32 + lane) * 2 + (i & 1)];
+                    add_window(cnt[r], track_window_pos<NW, CLAMP>(tc, p.ptab + (int64_t)i * p.n_pos, D, B));
+                }
+                npend[r] = 0;
+            }
+        }
+    }
+
+    // epilogue: threshold in bit-sliced form, emit the (rare) survivors
+    const int32_t tau = p.thr->tau_i;
+    const int pix = pg * 32 + lane;
+#pragma unroll
+    for (int r = 0; r < kPixTpl; ++r) {
+        if (!act[r] || pix >= p.n_pix) continue;
+        const uint64_t base =
+            ((((uint64_t)pix * p.n_ap + ia[r]) * p.n_P + ip) * p.n_tasc + it[r]) * (uint64_t)p.n_f0 + p.j0;
+        const Win<NW> ge = count_ge(cnt[r], tau);
+        int32_t *out = p.counts_full ? reinterpret_cast<int32_t *>(p.counts_full) + base : nullptr;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+            if (out) {
+                for (int bb = 0; bb < 32; ++bb)
+                    if (32 * w + bb < p.n_fj) out[32 * w + bb] = count_at(cnt[r], w, bb);
+            }
+            uint32_t m = ge.x[w] & valid_mask(p.n_fj, w);
+            while (m) {
+                const int bb = __ffs(m) - 1;
+                m &= m - 1;
+                const unsigned int pos = atomicAdd(p.cand_count, 1u);
+                if (pos < p.cand_cap) {
+                    RawCand rc;
+                    rc.index = base + 32 * w + bb;
+                    rc.key = (uint32_t)count_at(cnt[r], w, bb);
+                    rc.pad = 0u;
+                    p.cand[pos] = rc;
+                }
+            }
+        }
+    }
+}
+
+}  // namespace bsh
