@@ -230,6 +230,9 @@ def main_ours(args, rank, local_rank, world):
 
     # secondary: the weighted number count (FP32 weighted sum) on the same patch
     w_steps = max(1, min(args.steps, 5))
+    if args.no_weighted:
+        print(json.dumps({"profile_run": True, "unweighted_kernel_ms": float(np.mean(kern_ms))}), flush=True)
+        return
     w_total_ms, w_kern_ms, _, _ = timed(lambda: step(bsh.BSH_WEIGHTED), w_steps, 1)
     st_w = ctx.stats()
 
@@ -315,6 +318,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--profile", action="store_true",
                     help="only the timed unweighted + weighted steps (no e2e, no oracle): the command ncu wraps")
+    ap.add_argument("--no-weighted", action="store_true", help="with --profile: skip the weighted-count pass")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -70,7 +70,7 @@ struct bsh_ctx {
     std::string err;
     TableCache cache[2];
     uint64_t stamp = 0;
-    DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2, ptab, dpos, dpix;
+    DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2, ptab, dpos, dpix, psplit;
     DevBuf h_rho, h_w, h_peak, h_top;                  // device staging of bsh_search_patch_host
     unsigned int *pinned_count = nullptr;
     cudaEvent_t ev[10] = {};
@@ -252,12 +252,15 @@ int launch_stage1(bsh_ctx *ctx, K kernel, const P &p, int tpb, int grid, int sme
 
 int dispatch_unweighted(bsh_ctx *ctx, const Pending &pd, const Stage1Params &p, int grid)
 {
-    UNW_CASE(2, 6, 2, false) UNW_CASE(2, 6, 2, true) UNW_CASE(3, 6, 2, false) UNW_CASE(3, 6, 2, true)
+    UNW_CASE(3, 6, 2, false)
+#ifndef BSH_MINIMAL                                  /* tuning builds instantiate only the config-2 kernels */
+    UNW_CASE(2, 6, 2, false) UNW_CASE(2, 6, 2, true) UNW_CASE(3, 6, 2, true)
     UNW_CASE(2, 8, 2, false) UNW_CASE(2, 8, 2, true) UNW_CASE(3, 8, 2, false) UNW_CASE(3, 8, 2, true)
     UNW_CASE(2, 11, 2, false) UNW_CASE(2, 11, 2, true) UNW_CASE(3, 11, 2, false) UNW_CASE(3, 11, 2, true)
     UNW_CASE(2, 6, 1, false) UNW_CASE(3, 6, 1, false) UNW_CASE(2, 8, 1, false) UNW_CASE(3, 8, 1, false)
     UNW_CASE(2, 6, 1, true) UNW_CASE(3, 6, 1, true) UNW_CASE(2, 8, 1, true) UNW_CASE(3, 8, 1, true)
     UNW_CASE(2, 11, 1, false) UNW_CASE(3, 11, 1, false) UNW_CASE(2, 11, 1, true) UNW_CASE(3, 11, 1, true)
+#endif
     return fail(ctx, BSH_EINVAL, "no unweighted kernel for NW=%d HP=%d R=%d clamp=%d", pd.NW, pd.HP, pd.R, (int)pd.clamp);
 }
 
@@ -268,7 +271,10 @@ int dispatch_unweighted(bsh_ctx *ctx, const Pending &pd, const Stage1Params &p, 
 
 int dispatch_weighted(bsh_ctx *ctx, const Pending &pd, const Stage1Params &p, int grid)
 {
-    W_CASE(2, false) W_CASE(2, true) W_CASE(3, false) W_CASE(3, true)
+    W_CASE(3, false)
+#ifndef BSH_MINIMAL
+    W_CASE(2, false) W_CASE(2, true) W_CASE(3, true)
+#endif
     return fail(ctx, BSH_EINVAL, "no weighted kernel for NW=%d", pd.NW);
 }
 
@@ -278,9 +284,12 @@ int dispatch_weighted(bsh_ctx *ctx, const Pending &pd, const Stage1Params &p, in
 
 int dispatch_unweighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p, int grid)
 {
-    UNW_POS_CASE(2, 6, false) UNW_POS_CASE(2, 6, true) UNW_POS_CASE(3, 6, false) UNW_POS_CASE(3, 6, true)
+    UNW_POS_CASE(3, 6, false)
+#ifndef BSH_MINIMAL
+    UNW_POS_CASE(2, 6, false) UNW_POS_CASE(2, 6, true) UNW_POS_CASE(3, 6, true)
     UNW_POS_CASE(2, 8, false) UNW_POS_CASE(2, 8, true) UNW_POS_CASE(3, 8, false) UNW_POS_CASE(3, 8, true)
     UNW_POS_CASE(2, 11, false) UNW_POS_CASE(2, 11, true) UNW_POS_CASE(3, 11, false) UNW_POS_CASE(3, 11, true)
+#endif
     return fail(ctx, BSH_EINVAL, "no unweighted position kernel for NW=%d HP=%d clamp=%d", pd.NW, pd.HP, (int)pd.clamp);
 }
 
@@ -290,9 +299,12 @@ int dispatch_unweighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p,
 
 int dispatch_unweighted_pix(bsh_ctx *ctx, const Pending &pd, const PixParams &p, int grid)
 {
-    UNW_PIX_CASE(2, 6, false) UNW_PIX_CASE(2, 6, true) UNW_PIX_CASE(3, 6, false) UNW_PIX_CASE(3, 6, true)
+    UNW_PIX_CASE(3, 6, false)
+#ifndef BSH_MINIMAL
+    UNW_PIX_CASE(2, 6, false) UNW_PIX_CASE(2, 6, true) UNW_PIX_CASE(3, 6, true)
     UNW_PIX_CASE(2, 8, false) UNW_PIX_CASE(2, 8, true) UNW_PIX_CASE(3, 8, false) UNW_PIX_CASE(3, 8, true)
     UNW_PIX_CASE(2, 11, false) UNW_PIX_CASE(2, 11, true) UNW_PIX_CASE(3, 11, false) UNW_PIX_CASE(3, 11, true)
+#endif
     return fail(ctx, BSH_EINVAL, "no unweighted pixel-lane kernel for NW=%d HP=%d clamp=%d", pd.NW, pd.HP, (int)pd.clamp);
 }
 
@@ -303,8 +315,11 @@ int dispatch_unweighted_pix(bsh_ctx *ctx, const Pending &pd, const PixParams &p,
 int dispatch_weighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p, int grid)
 {
     const int nb = pd.NW == 2 ? 64 : (p.n_fj <= 90 ? 90 : 96);
-    W_POS_CASE(2, 64, false) W_POS_CASE(2, 64, true) W_POS_CASE(3, 90, false) W_POS_CASE(3, 90, true)
+    W_POS_CASE(3, 90, false)
+#ifndef BSH_MINIMAL
+    W_POS_CASE(2, 64, false) W_POS_CASE(2, 64, true) W_POS_CASE(3, 90, true)
     W_POS_CASE(3, 96, false) W_POS_CASE(3, 96, true)
+#endif
     return fail(ctx, BSH_EINVAL, "no weighted position kernel for NW=%d", pd.NW);
 }
 
@@ -341,6 +356,7 @@ int run_pass(bsh_ctx *ctx)
             p.ptab = (const uint4 *)ctx->ptab.p;
             p.cs = (const double2 *)c.d_cs.p;
             p.dpix = (const double *)ctx->dpix.p;
+            p.split = (const unsigned char *)ctx->psplit.p;
             p.A = (const double *)c.d_A.p;
             p.casa = (const double2 *)c.d_casa.p;
             p.n_pad = pd.n_pad; p.n_pos = pd.n_pos; p.n_chunks = pd.n_pad / kStageSfts; p.n_stages = pd.pix_stages;
@@ -486,7 +502,7 @@ int bsh_destroy(bsh_ctx *ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf *bufs[] = {&ctx->wtab, &ctx->w_pad, &ctx->stats, &ctx->thr, &ctx->dtab, &ctx->nvec, &ctx->cand, &ctx->cand_count,
-                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top};
+                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->psplit, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto &c : ctx->cache) {
@@ -617,6 +633,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
                      getenv("BSH_LEGACY") == nullptr && getenv("BSH_NO_PIX") == nullptr && !(mode & BSH_NAIVE);
         pd.pix_stages = std::max(1, std::min(pd.pix_stages, pd.n_pad / kStageSfts));
         pd.pix_smem = kPixHeader + pd.pix_stages * ps.stride;
+        if (const char *e = getenv("BSH_SMEM_PAD")) pd.pix_smem += atoi(e);              // tuning: lowers the occupancy
     }
     pd.emit_all = pd.n_templates <= kCandCap;
     pd.frac = (double)std::max<int64_t>(8ll * topk, 4096) / (double)pd.n_templates;
@@ -647,6 +664,10 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         build_position_table_kernel<<<(unsigned)((n_ent + 255) / 256), 256, 0, ctx->stream>>>(
             d_peak, words_per_row, sfts->n_sft, pd.n_pad, sfts->n_bins, pd.n_pos, pd.pos_off, pd.pos_s_zero,
             (uint4 *)ctx->ptab.p);
+        count_launch(ctx);
+        TRY(ensure(ctx, ctx->psplit, (size_t)pd.n_pad * pd.n_pos * 12));
+        split_position_table_kernel<<<(unsigned)((n_ent + 255) / 256), 256, 0, ctx->stream>>>(
+            (const uint4 *)ctx->ptab.p, pd.n_pad, pd.n_pos, (unsigned char *)ctx->psplit.p);
         count_launch(ctx);
         const int64_t n_d = (int64_t)pd.n_pg * pd.n_pad * 32;
         dtable_pix_kernel<<<(unsigned)((n_d + 255) / 256), 256, 0, ctx->stream>>>(

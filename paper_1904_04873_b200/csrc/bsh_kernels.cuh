@@ -47,6 +47,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "WAIT_LOOP:\n\t"
         "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
         "@P1 bra WAIT_DONE;\n\t"
+#ifdef BSH_WAIT_SLEEP
+        "nanosleep.u32 64;\n\t"
+#endif
         "bra WAIT_LOOP;\n\t"
         "WAIT_DONE:\n\t"
         "}" ::"r"(smem_u32(bar)),

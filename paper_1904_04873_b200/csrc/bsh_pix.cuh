@@ -58,8 +58,27 @@ __global__ void __launch_bounds__(256) dtable_pix_kernel(const double *__restric
     dpix[t] = D;
 }
 
+// Split position table staged by the pixel-lane kernel: per stage of kStageSfts SFTs, first the (word 0, word 1) pairs
+// [kk][p] (8 bytes each), then the words 2 [kk][p] (4 bytes each).  The window of a position is then read with one
+// LDS.64 and one LDS.32 from two different arrays (12 bytes, 3 shared-memory wavefronts per warp) -- a 16-byte entry
+// would be fetched as one LDS.128 (4 wavefronts) whatever the source says, ptxas fuses adjacent reads.
+__global__ void __launch_bounds__(256) split_position_table_kernel(const uint4 *__restrict__ ptab, int n_pad, int n_pos,
+                                                                   unsigned char *__restrict__ split)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (int64_t)n_pad * n_pos) return;
+    const int i = (int)(t / n_pos), p = (int)(t % n_pos);
+    const uint4 e = ptab[t];
+    const int64_t stage_bytes = (int64_t)kStageSfts * n_pos * 12;
+    unsigned char *base = split + (int64_t)(i / kStageSfts) * stage_bytes;
+    const int kk = i % kStageSfts;
+    reinterpret_cast<uint2 *>(base)[kk * n_pos + p] = make_uint2(e.x, e.y);
+    reinterpret_cast<uint32_t *>(base + (int64_t)kStageSfts * n_pos * 8)[kk * n_pos + p] = e.z;
+}
+
 struct PixParams {
-    const uint4 *ptab;          // [n_pad][n_pos]
+    const uint4 *ptab;          // [n_pad][n_pos]  (fix-ups)
+    const unsigned char *split; // [n_pad / kStageSfts] stages of the split table (hot loop)
     const double2 *cs;          // [n_P][n_pad]  (cos, sin)(Omega_p t_i)
     const double *dpix;         // [n_pg][n_pad / 2][32][2]
     const double *A;            // [n_ap][n_P]
@@ -81,7 +100,7 @@ struct PixStage {
     int tab_bytes, cs_bytes, d_bytes, stride;
     __device__ __host__ PixStage(int n_pos)
     {
-        tab_bytes = kStageSfts * n_pos * 16;
+        tab_bytes = kStageSfts * n_pos * 12;
         cs_bytes = kStageSfts * 16;
         d_bytes = kStageSfts * 32 * 8;
         stride = tab_bytes + cs_bytes + d_bytes;
@@ -94,7 +113,7 @@ __device__ __forceinline__ void pix_issue(const PixParams &p, const PixStage &L,
 {
     const int64_t i0 = (int64_t)chunk * kStageSfts;
     mbar_expect_tx(bar, (uint32_t)L.stride);
-    tma_bulk_g2s(stage, p.ptab + i0 * p.n_pos, (uint32_t)L.tab_bytes, bar);
+    tma_bulk_g2s(stage, p.split + (int64_t)chunk * L.tab_bytes, (uint32_t)L.tab_bytes, bar);
     tma_bulk_g2s(stage + L.tab_bytes, p.cs + (int64_t)ip * p.n_pad + i0, (uint32_t)L.cs_bytes, bar);
     tma_bulk_g2s(stage + L.tab_bytes + L.cs_bytes, p.dpix + ((int64_t)pg * p.n_pad + i0) * 32, (uint32_t)L.d_bytes, bar);
 }
@@ -140,9 +159,21 @@ __device__ __forceinline__ int32_t pix_position(const PixConst &k, double D, dou
     return brk ? k.s_zero : s0;
 }
 
+// Window of position s of stage row kk: words 0, 1 from the pair array, word 2 from the word array.
+template <int NW>
+__device__ __forceinline__ Win<NW> pix_load(const unsigned char *tab, int n_pos, int kk, int32_t s)
+{
+    Win<NW> w;
+    const uint2 lo = reinterpret_cast<const uint2 *>(tab)[kk * n_pos + s];
+    w.x[0] = lo.x;
+    if (NW > 1) w.x[1 % NW] = lo.y;
+    if (NW > 2) w.x[2 % NW] = reinterpret_cast<const uint32_t *>(tab + kStageSfts * n_pos * 8)[kk * n_pos + s];
+    return w;
+}
+
 // One SFT (slot K of the unrolled block of 32) for both templates of the thread.
 template <int K, int NW, int HP, bool CLAMP>
-__device__ __forceinline__ void pix_step(const PixConst &k, const uint4 *tab, int n_pos, const double2 *bpair,
+__device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char *tab, int n_pos, const double2 *bpair,
                                          const double2 *dpair, Counter<NW, HP> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl])
 {
     constexpr int kk = K % kStageSfts;
@@ -155,20 +186,23 @@ __device__ __forceinline__ void pix_step(const PixConst &k, const uint4 *tab, in
         bool b;
         const int32_t s = pix_position<CLAMP>(k, D, Bv[r], b);
         brk[r] |= b ? (1u << K) : 0u;
-        push<K, NW, HP>(cnt[r], load_position<NW>(tab + kk * n_pos, s));
+        push<K, NW, HP>(cnt[r], pix_load<NW>(tab, n_pos, kk, s));
     }
 }
 
 template <int K0, int NW, int HP, bool CLAMP, int... Ks>
-__device__ __forceinline__ void pix_half(const PixConst &k, const uint4 *tab, int n_pos, const double2 *bpair,
+__device__ __forceinline__ void pix_half(const PixConst &k, const unsigned char *tab, int n_pos, const double2 *bpair,
                                          const double2 *dpair, Counter<NW, HP> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl],
                                          std::integer_sequence<int, Ks...>)
 {
     (pix_step<K0 + Ks, NW, HP, CLAMP>(k, tab, n_pos, bpair, dpair, cnt, brk), ...);
 }
 
+#ifndef BSH_PIX_MINB
+#define BSH_PIX_MINB 2
+#endif
 template <int NW, int HP, bool CLAMP>
-__global__ void __launch_bounds__(32 * kPixWarps, 2) stage1_unweighted_pix_kernel(const PixParams p)
+__global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighted_pix_kernel(const PixParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);
@@ -251,10 +285,10 @@ __global__ void __launch_bounds__(32 * kPixWarps, 2) stage1_unweighted_pix_kerne
             const double2 *bpair = reinterpret_cast<const double2 *>(bbuf + half * 32);
             const double2 *dpair = reinterpret_cast<const double2 *>(sp + L.tab_bytes + L.cs_bytes) + lane;
             if (half == 0)
-                pix_half<0, NW, HP, CLAMP>(kc, reinterpret_cast<const uint4 *>(sp), p.n_pos, bpair, dpair, cnt, brk,
+                pix_half<0, NW, HP, CLAMP>(kc, sp, p.n_pos, bpair, dpair, cnt, brk,
                                            std::make_integer_sequence<int, kStageSfts>{});
             else
-                pix_half<kStageSfts, NW, HP, CLAMP>(kc, reinterpret_cast<const uint4 *>(sp), p.n_pos, bpair, dpair, cnt, brk,
+                pix_half<kStageSfts, NW, HP, CLAMP>(kc, sp, p.n_pos, bpair, dpair, cnt, brk,
                                                     std::make_integer_sequence<int, kStageSfts>{});
             pix_release(p, L, smem, st, 2 * blk + half, lane, ip, pg);
             if (++st == p.n_stages) { st = 0; parity ^= 1u; }
