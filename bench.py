@@ -33,19 +33,26 @@ METRIC = "template*SFT Hough accumulations/sec"
 UNIT = "accumulations/s"
 
 # --- roofline model of the stage-1 accumulation kernel -----------------------------------------
+# Unit of work: one (pixel, binary template, SFT) TRIPLE = n_f0 (90) accumulations.  The kernel is bound on chip, by the
+# shared-memory data pipe (north_star's bound (b); ncu: l1tex__data_pipe_lsu_wavefronts is the busiest unit).
 N_SM = 148
-LANES_PER_SM_CLK = 128            # 4 SMSPs x 32 lanes: warp-instruction issue peak
-# algorithmic lane-operations per (pixel, binary template, SFT) triple, i.e. per 90 accumulations:
-#   FP64: g = D - B (1), y at both band ends (2), + 1/2 (2), floor via magic add (2), binary term A(C CA + S SA) shared by
-#         the 2 pixels of a thread (4 / 2)                                                              -> 9
-#   INT : 3 funnel shifts (window), 6 LOP3 (3 full adders), high-plane ripple 2*3*HP/32, address 2       -> 12.1 (HP = 6)
-#   LSU : one 16-byte window load + shared (cos, sin) and D loads (2 / 2)                                -> 2
-OPS_PER_TRIPLE_UNWEIGHTED = 9.0 + 12.1 + 2.0
-# weighted: the same track + window work with 1 pixel per thread (7 + 4 FP64, 3 + 2 INT, 3 LSU) plus one predicated FP32
-# add and one predicate-generating op per accumulation
+SMEM_BYTES_PER_CLK_SM = 128       # one 128-byte wavefront per clock per SM (B300_MICROARCH.md "smem crossbar BW";
+                                  # confirmed with an LDS microbenchmark under ncu on this pool)
+# algorithmic shared-memory bytes per triple: the gathered 96-bit window of the 90 f0 bins (12 B), the Doppler term D of
+# the (pixel, SFT) shared by the 2 templates of a thread (8 / 2 B) and the binary term B of the (template, SFT), one
+# 128-byte wavefront per 2 templates x 32 pixels (4 B per triple)
+SMEM_BYTES_PER_TRIPLE = 12.0 + 4.0 + 4.0
+# secondary view, integer-ALU pipe: 2 LOP3 per window word (carry-save full adder) x 3 words + ripple into the 6 high
+# planes once per 32 SFTs (2 x 3 x 6 / 32): the part of the count that cannot be moved to another pipe
+ALU_LANES_PER_SM_CLK = 64         # 16 lanes/clk/SMSP (B300_MICROARCH.md: alu-pipe rt_SMSP = 2)
+ALU_OPS_PER_TRIPLE = 6.0 + 1.125
+LANES_PER_SM_CLK = 128            # warp-instruction issue peak
+# weighted kernel: one predicated FP32 add + one predicate-generating op per accumulation, plus the track per triple
 OPS_PER_TRIPLE_WEIGHTED_FIXED = 19.0
 OPS_PER_ACC_WEIGHTED = 2.0
-GATHER_LANES_PER_SM_CLK = 32      # north_star bound (b): one shared-memory lane-gather per accumulation
+GATHER_LANES_PER_SM_CLK = 32      # north_star bound (b) read literally: one 4-byte lane-gather per accumulation
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the kernel (ncu --set full, profiles/r01c_stage1_pix_full.md)
+NCU_DRAM_BYTES_PER_LAUNCH = None
 
 
 def measured_peaks():
@@ -164,6 +171,7 @@ def main_reference(args, rank, world):
 def main_ours(args, rank, local_rank, world):
     import torch
     import paper_1904_04873_b200 as bsh
+    from paper_1904_04873_b200 import sharding
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
@@ -214,10 +222,7 @@ def main_ours(args, rank, local_rank, world):
             dist.barrier()
         total_ms = sum(a.elapsed_time(b) for a, b in ev)
         launches = ctx.stats()["launches"] - l0
-        if dist:
-            t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            total_ms = float(t.item())
+        total_ms = sharding.max_over_ranks(total_ms, dist)
         return total_ms, kern_ms, launches, wall
 
     sampler = ClockSampler(physical_gpu_index(local_rank))
@@ -257,11 +262,16 @@ def main_ours(args, rank, local_rank, world):
     k_ms = float(np.mean(kern_ms))
     triples = wl.n_pix * wl.n_binary * wl.n_sft
     issue_peak = N_SM * LANES_PER_SM_CLK * sm_max * 1e6 / 1e12                    # Tlaneop/s
-    achieved = triples * OPS_PER_TRIPLE_UNWEIGHTED / (k_ms * 1e-3) / 1e12
+    smem_peak = N_SM * SMEM_BYTES_PER_CLK_SM * sm_max * 1e6 / 1e9                 # GB/s
+    smem_achieved = triples * SMEM_BYTES_PER_TRIPLE / (k_ms * 1e-3) / 1e9
+    alu_peak = N_SM * ALU_LANES_PER_SM_CLK * sm_max * 1e6 / 1e12
+    alu_achieved = triples * ALU_OPS_PER_TRIPLE / (k_ms * 1e-3) / 1e12
     gather_peak = N_SM * GATHER_LANES_PER_SM_CLK * sm_max * 1e6
     wk_ms = float(np.mean(w_kern_ms))
     w_ops = triples * OPS_PER_TRIPLE_WEIGHTED_FIXED + wl.n_accumulations * OPS_PER_ACC_WEIGHTED
     cpu_value, _, cores, sample = run_oracle_steps(wl, 1, 0, seconds_per_step=15.0)
+    kname = {2: "stage1_unweighted_pix_kernel", 1: "stage1_unweighted_pos_kernel"}.get(st["kernel_variant"] // 1000,
+                                                                                       "stage1_unweighted_kernel")
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -277,22 +287,26 @@ def main_ours(args, rank, local_rank, world):
                 "d2h_bytes_per_step": int(h_out.numel()), "ms_per_step": e_total_ms / args.steps,
                 "call": "bsh_search_patch_host (pinned host buffers)"},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "alu", "kernel": "stage1_unweighted_kernel", "achieved": achieved, "peak": issue_peak,
-                     "unit": "Tlaneop/s", "frac": achieved / issue_peak, "traffic": None,
+        "roofline": {"bound": "smem", "kernel": kname, "achieved": smem_achieved, "peak": smem_peak, "unit": "GB/s",
+                     "frac": smem_achieved / smem_peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
                      "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (total_ms / args.steps),
-                     "ops_per_triple": OPS_PER_TRIPLE_UNWEIGHTED, "triples_per_launch": triples,
-                     "peak_source": f"148 SMs x 128 lanes/clk x {sm_max:.0f} MHz (B200_PROFILING.md unit counts; "
-                                    "MEASURED_PEAKS.json holds only HBM and bf16 peaks)",
-                     "gather_bound": {"note": "north_star bound (b): one shared-memory lane-gather per accumulation at "
-                                              "32 lanes/clk/SM; > 1 because 90 f0 bins share each gathered word",
+                     "bytes_per_triple": SMEM_BYTES_PER_TRIPLE, "triples_per_launch": triples,
+                     "peak_source": f"shared-memory data pipe: 148 SMs x 128 B/clk x {sm_max:.0f} MHz (guide unit counts "
+                                    "and clock; MEASURED_PEAKS.json holds only HBM and bf16 peaks, and HBM is not the "
+                                    "bound: ~3 MB of tables per launch)",
+                     "alu_view": {"ops_per_triple": ALU_OPS_PER_TRIPLE, "achieved_tlaneops": alu_achieved,
+                                  "peak_tlaneops": alu_peak, "frac": alu_achieved / alu_peak},
+                     "gather_bound": {"note": "north_star bound (b) read literally: one 4-byte shared-memory lane-gather "
+                                              "per accumulation at 32 lanes/clk/SM; > 1 because the 90 f0 bins of a band "
+                                              "share each gathered window",
                                       "achieved_gathers_per_s": acc_per_step / (k_ms * 1e-3), "peak": gather_peak,
                                       "frac": acc_per_step / (k_ms * 1e-3) / gather_peak},
-                     "hbm_bound": {"bytes_per_launch": int(st["n_accumulations"] and (wl.n_sft * 6 * 16 + 30 * wl.n_sft * 16
-                                                                                    + 64 * wl.n_sft * 8)),
-                                   "note": "slab + tables are ~2.5 MB per patch: HBM time ~0.4 us, never the bound"}},
+                     "hbm_bound": {"note": "position table + (cos, sin) + D tables are ~3 MB per patch, read once from "
+                                           "DRAM then served by L2: ~0.5 us at the measured HBM rate, never the bound",
+                                   "hbm_gbs_measured": peaks.get("hbm_gbs")}},
         "weighted": {"value": world * w_steps * acc_per_step / (w_total_ms * 1e-3), "unit": UNIT,
                      "ms_per_step": w_total_ms / w_steps, "kernel_ms": wk_ms, "kernel": "stage1_weighted_kernel",
-                     "roofline_frac_alu": w_ops / (wk_ms * 1e-3) / 1e12 / issue_peak, "n_passes": st_w["n_passes"]},
+                     "roofline_frac_issue": w_ops / (wk_ms * 1e-3) / 1e12 / issue_peak, "n_passes": st_w["n_passes"]},
         "stage_ms": {"peakgram": st["peakgram_ms"], "stage1_setup": st["stage1_setup_ms"], "stage1_kernel": k_ms,
                      "stage1_select": st["stage1_select_ms"], "stage2": st["stage2_ms"]},
         "stage1": {"n_candidates": st["n_candidates"], "threshold": st["threshold"], "n_passes": st["n_passes"],

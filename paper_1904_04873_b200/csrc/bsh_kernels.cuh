@@ -45,11 +45,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "{\n\t"
         ".reg .pred P1;\n\t"
         "WAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"   // plain polling: a suspend-time hint or a
+                                                                          // nanosleep back-off measured 5-10 % slower
         "@P1 bra WAIT_DONE;\n\t"
-#ifdef BSH_WAIT_SLEEP
-        "nanosleep.u32 64;\n\t"
-#endif
         "bra WAIT_LOOP;\n\t"
         "WAIT_DONE:\n\t"
         "}" ::"r"(smem_u32(bar)),

@@ -22,7 +22,7 @@
 namespace bsh {
 
 constexpr int kStageSfts = 16;        // SFTs per shared-memory stage (half an unrolled block of 32)
-constexpr int kMaxStages = 4;
+constexpr int kMaxStages = 6;
 constexpr int kPosHeader = 128;       // full[kMaxStages] mbarriers + done[kMaxStages] counters
 constexpr int kListCap = 64;          // deferred breaks per (thread, pixel); flushed when more than 32 are pending
 constexpr int kWarpsUnweighted = 8;   // warps per block = pixel groups per block
