@@ -33,26 +33,29 @@ METRIC = "template*SFT Hough accumulations/sec"
 UNIT = "accumulations/s"
 
 # --- roofline model of the stage-1 accumulation kernel -----------------------------------------
-# Unit of work: one (pixel, binary template, SFT) TRIPLE = n_f0 (90) accumulations.  The kernel is bound on chip, by the
-# shared-memory data pipe (north_star's bound (b); ncu: l1tex__data_pipe_lsu_wavefronts is the busiest unit).
+# Unit of work: one (pixel, binary template, SFT) TRIPLE = n_f0 (90) accumulations.  The kernel is bound on chip by plain
+# instruction throughput: every pipe it uses (integer ALU, FP64, LSU/shared memory) is 40-60 % busy and the warp
+# schedulers issue 63 % of their slots (ncu, profiles/r01c_stage1_pix_full.md); HBM is idle.  Roofline = warp-issue peak.
 N_SM = 148
-SMEM_BYTES_PER_CLK_SM = 128       # one 128-byte wavefront per clock per SM (B300_MICROARCH.md "smem crossbar BW";
-                                  # confirmed with an LDS microbenchmark under ncu on this pool)
-# algorithmic shared-memory bytes per triple: the gathered 96-bit window of the 90 f0 bins (12 B), the Doppler term D of
-# the (pixel, SFT) shared by the 2 templates of a thread (8 / 2 B) and the binary term B of the (template, SFT), one
-# 128-byte wavefront per 2 templates x 32 pixels (4 B per triple)
-SMEM_BYTES_PER_TRIPLE = 12.0 + 4.0 + 4.0
-# secondary view, integer-ALU pipe: 2 LOP3 per window word (carry-save full adder) x 3 words + ripple into the 6 high
-# planes once per 32 SFTs (2 x 3 x 6 / 32): the part of the count that cannot be moved to another pipe
-ALU_LANES_PER_SM_CLK = 64         # 16 lanes/clk/SMSP (B300_MICROARCH.md: alu-pipe rt_SMSP = 2)
-ALU_OPS_PER_TRIPLE = 6.0 + 1.125
-LANES_PER_SM_CLK = 128            # warp-instruction issue peak
+LANES_PER_SM_CLK = 128            # 4 SMSPs x 32 lanes: one warp instruction per scheduler per clock
+# algorithmic lane-instructions per triple -- what this formulation must execute whatever the schedule:
+#   FP64  g = D - B (1), y at both band ends (2), + 1/2 (2), floor by magic add (2), equal-shift test (1)           8
+#   count 3 window words x full adder (2 LOP3) + ripple into the 6 high planes once per 32 SFTs (36 / 32)           7.125
+#   INT   position select on a break (1), break mask (1), shared-memory address (1)                                 3
+#   LSU   window read (LDS.64 + LDS.32) 2, binary terms of 2 templates per load 0.5, Doppler terms of 2 SFTs
+#         per load shared by 2 templates 0.25                                                                       2.75
+ALGO_OPS_PER_TRIPLE = 8.0 + 7.125 + 3.0 + 2.75
+# secondary views: the shared-memory data pipe (one 128-byte wavefront per clock per SM) and the integer-ALU pipe alone
+SMEM_BYTES_PER_CLK_SM = 128
+SMEM_BYTES_PER_TRIPLE = 12.0 + 4.0 + 4.0      # 96-bit window + D (8 B per 2 templates) + B (one wavefront per 32 triples)
+ALU_LANES_PER_SM_CLK = 64                      # 16 lanes/clk/SMSP (B300_MICROARCH.md: alu-pipe rt_SMSP = 2)
+ALU_OPS_PER_TRIPLE = 6.0 + 1.125 + 3.0
 # weighted kernel: one predicated FP32 add + one predicate-generating op per accumulation, plus the track per triple
 OPS_PER_TRIPLE_WEIGHTED_FIXED = 19.0
 OPS_PER_ACC_WEIGHTED = 2.0
 GATHER_LANES_PER_SM_CLK = 32      # north_star bound (b) read literally: one 4-byte lane-gather per accumulation
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the kernel (ncu --set full, profiles/r01c_stage1_pix_full.md)
-NCU_DRAM_BYTES_PER_LAUNCH = None
+NCU_DRAM_BYTES_PER_LAUNCH = 12731648 + 747520
 
 
 def measured_peaks():
@@ -266,6 +269,7 @@ def main_ours(args, rank, local_rank, world):
     smem_achieved = triples * SMEM_BYTES_PER_TRIPLE / (k_ms * 1e-3) / 1e9
     alu_peak = N_SM * ALU_LANES_PER_SM_CLK * sm_max * 1e6 / 1e12
     alu_achieved = triples * ALU_OPS_PER_TRIPLE / (k_ms * 1e-3) / 1e12
+    algo_achieved = triples * ALGO_OPS_PER_TRIPLE / (k_ms * 1e-3) / 1e12
     gather_peak = N_SM * GATHER_LANES_PER_SM_CLK * sm_max * 1e6
     wk_ms = float(np.mean(w_kern_ms))
     w_ops = triples * OPS_PER_TRIPLE_WEIGHTED_FIXED + wl.n_accumulations * OPS_PER_ACC_WEIGHTED
@@ -287,15 +291,17 @@ def main_ours(args, rank, local_rank, world):
                 "d2h_bytes_per_step": int(h_out.numel()), "ms_per_step": e_total_ms / args.steps,
                 "call": "bsh_search_patch_host (pinned host buffers)"},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "smem", "kernel": kname, "achieved": smem_achieved, "peak": smem_peak, "unit": "GB/s",
-                     "frac": smem_achieved / smem_peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+        "roofline": {"bound": "alu", "kernel": kname, "achieved": algo_achieved, "peak": issue_peak, "unit": "Tlaneop/s",
+                     "frac": algo_achieved / issue_peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
                      "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (total_ms / args.steps),
-                     "bytes_per_triple": SMEM_BYTES_PER_TRIPLE, "triples_per_launch": triples,
-                     "peak_source": f"shared-memory data pipe: 148 SMs x 128 B/clk x {sm_max:.0f} MHz (guide unit counts "
-                                    "and clock; MEASURED_PEAKS.json holds only HBM and bf16 peaks, and HBM is not the "
-                                    "bound: ~3 MB of tables per launch)",
-                     "alu_view": {"ops_per_triple": ALU_OPS_PER_TRIPLE, "achieved_tlaneops": alu_achieved,
-                                  "peak_tlaneops": alu_peak, "frac": alu_achieved / alu_peak},
+                     "ops_per_triple": ALGO_OPS_PER_TRIPLE, "triples_per_launch": triples,
+                     "peak_source": f"warp-issue peak: 148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz (guide unit counts "
+                                    "and clock; MEASURED_PEAKS.json holds only HBM and bf16 peaks, and HBM is idle here: "
+                                    "13.5 MB of DRAM traffic per launch)",
+                     "smem_view": {"bytes_per_triple": SMEM_BYTES_PER_TRIPLE, "achieved_gbs": smem_achieved,
+                                   "peak_gbs": smem_peak, "frac": smem_achieved / smem_peak},
+                     "alu_pipe_view": {"ops_per_triple": ALU_OPS_PER_TRIPLE, "achieved_tlaneops": alu_achieved,
+                                       "peak_tlaneops": alu_peak, "frac": alu_achieved / alu_peak},
                      "gather_bound": {"note": "north_star bound (b) read literally: one 4-byte shared-memory lane-gather "
                                               "per accumulation at 32 lanes/clk/SM; > 1 because the 90 f0 bins of a band "
                                               "share each gathered window",

@@ -197,6 +197,41 @@ def test_multiple_breaks_per_band_fallback(bsh, torch, ctx):
 
 
 # ------------------------------------------------------------------------------------------------------------
+# the pixel-lane kernel (bsh_pix.cuh) forced on small and ragged problems: partly filled pixel groups (1, 9, 36 pixels),
+# several f0 tiles with a ragged last one, SFT counts off the 32-block, both table geometries, the multi-break fallback
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_sft,n_f0,margin,f0,side", [(1, 1, 3, 50.0, 1), (33, 7, 12, 80.0, 3), (64, 90, 30, 120.0, 6),
+                                                        (130, 97, 45, 150.0, 6), (70, 200, 60, 200.0, 3),
+                                                        (2100, 64, 50, 180.0, 6)])
+def test_pixel_lane_kernel_ragged(bsh, torch, ctx, monkeypatch, n_sft, n_f0, margin, f0, side):
+    wl = synth.noise_workload(seed=1000 + n_sft + n_f0, n_sft=n_sft, n_f0=n_f0, margin=margin, f_band_start=f0,
+                              n_pix_side=side, ap=(10.0, 40.0), P_days=(15.0, 31.0), n_t=3, topk=7)
+    pk = oracle.peakgram(wl.rho)
+    want_n, _ = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL, want_wcount=False)
+    monkeypatch.setenv("BSH_FORCE_PIX", "1")
+    for force_clamp in (False, True):
+        if force_clamp:
+            monkeypatch.setenv("BSH_FORCE_CLAMP", "1")
+        else:
+            monkeypatch.delenv("BSH_FORCE_CLAMP", raising=False)
+        r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
+        assert ctx.stats()["kernel_variant"] // 1000 == 2, "the pixel-lane kernel did not run"
+        assert np.array_equal(r["counts"], want_n), force_clamp
+        check_unweighted_toplist(r["top"], want_n, 7)
+
+
+def test_pixel_lane_kernel_multiple_breaks(bsh, torch, ctx, monkeypatch):
+    wl = synth.noise_workload(seed=78, n_sft=96, n_f0=90, margin=40, f_band_start=150.0, n_pix_side=2,
+                              ap=(2500.0, 6000.0), P_days=(15.0,), n_t=4)
+    pk = oracle.peakgram(wl.rho)
+    want_n, _ = oracle.stage1(wl, pk, None, mode=oracle.CANONICAL)
+    monkeypatch.setenv("BSH_FORCE_PIX", "1")
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
+    assert ctx.stats()["kernel_variant"] // 1000 == 2
+    assert np.array_equal(r["counts"], want_n)
+
+
+# ------------------------------------------------------------------------------------------------------------
 # config 2: a complete sub-grid element by element, then the full grid in the bench's launch configuration
 # ------------------------------------------------------------------------------------------------------------
 def test_config2_subgrid_element_by_element(bsh, torch, ctx):
