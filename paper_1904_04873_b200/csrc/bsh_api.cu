@@ -51,6 +51,7 @@ struct Pending {                      // state between bsh_stage1_launch and bsh
     int64_t k_band0 = 0, k_slab0 = 0;
     uint64_t n_templates = 0;
     bool emit_all = false, clamp = false;
+    int tile_bins = 96;               // f0 bins per accumulation pass (<= 32 NW)
     int R = 2, NW = 3, HP = 6, n_entries = 0, off_table = 0, s_max = 0, s_zero = 0, list_cap = 0, tpb = 256, n_groups = 0, n_aq_tiles = 0;
     double frac = 0, shift_sigma = 0;
     int passes = 0;
@@ -314,10 +315,10 @@ int dispatch_unweighted_pix(bsh_ctx *ctx, const Pending &pd, const PixParams &p,
 
 int dispatch_weighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p, int grid)
 {
-    const int nb = pd.NW == 2 ? 64 : (p.n_fj <= 90 ? 90 : 96);
-    W_POS_CASE(3, 90, false)
+    const int nb = pd.NW == 2 ? (pd.tile_bins <= 48 ? 48 : 64) : (p.n_fj <= 90 ? 90 : 96);
+    W_POS_CASE(3, 90, false) W_POS_CASE(2, 48, false)
 #ifndef BSH_MINIMAL
-    W_POS_CASE(2, 64, false) W_POS_CASE(2, 64, true) W_POS_CASE(3, 90, true)
+    W_POS_CASE(2, 64, false) W_POS_CASE(2, 64, true) W_POS_CASE(3, 90, true) W_POS_CASE(2, 48, true)
     W_POS_CASE(3, 96, false) W_POS_CASE(3, 96, true)
 #endif
     return fail(ctx, BSH_EINVAL, "no weighted position kernel for NW=%d", pd.NW);
@@ -350,7 +351,7 @@ int run_pass(bsh_ctx *ctx)
         ctx->st.grid_blocks = (int)blocks;
         ctx->st.threads_per_block = 256;
     } else if (pd.use_pix && !weighted) {
-        const int tile_bins = 32 * pd.NW;
+        const int tile_bins = pd.tile_bins;
         for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
             PixParams p;
             p.ptab = (const uint4 *)ctx->ptab.p;
@@ -379,7 +380,7 @@ int run_pass(bsh_ctx *ctx)
             TRY(dispatch_unweighted_pix(ctx, pd, p, (int)grid));
         }
     } else if (pd.use_pos) {
-        const int tile_bins = 32 * pd.NW;
+        const int tile_bins = pd.tile_bins;
         for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
             PosParams p;
             p.ptab = (const uint4 *)ctx->ptab.p;
@@ -408,7 +409,7 @@ int run_pass(bsh_ctx *ctx)
             TRY(weighted ? dispatch_weighted_pos(ctx, pd, p, (int)grid) : dispatch_unweighted_pos(ctx, pd, p, (int)grid));
         }
     } else {
-        const int tile_bins = 32 * pd.NW;
+        const int tile_bins = pd.tile_bins;
         for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
             Stage1Params p;
             p.wtab = (const uint4 *)ctx->wtab.p;
@@ -589,6 +590,13 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     // kernel shape
     pd.NW = grid->n_f0 <= 64 ? 2 : 3;
     pd.R = weighted ? 1 : 2;
+    pd.tile_bins = 32 * pd.NW;
+    // weighted count: one FP32 accumulator per bin lives in registers; 90 of them spill (ncu: 0.2 local-memory accesses
+    // per accumulation), so a band of 65..96 bins is done as two passes of half the bins (two-word windows)
+    if (weighted && grid->n_f0 > 64 && grid->n_f0 <= 96 && getenv("BSH_W_FULLTILE") == nullptr) {
+        pd.NW = 2;
+        pd.tile_bins = (grid->n_f0 + 1) / 2;
+    }
     if (const char *e = getenv("BSH_PIXELS_PER_THREAD")) {
         const int r = atoi(e);
         if (!weighted && (r == 1 || r == 2)) pd.R = r;
@@ -608,12 +616,12 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     if (const char *e = getenv("BSH_LIST_CAP")) pd.list_cap = std::max(1, atoi(e));
     pd.n_groups = (grid->n_pix + pd.R - 1) / pd.R;
     {   // position-table kernels when 2+ stages of the table fit in shared memory (else the funnel-shift kernels)
-        const PosGeometry pg = pos_geometry(tg, sfts->n_bins, grid->n_f0, pd.NW);
+        const PosGeometry pg = pos_geometry(tg, sfts->n_bins, grid->n_f0, pd.NW, pd.tile_bins);
         pd.pos_off = pg.off_table; pd.pos_s_max = pg.s_max; pd.pos_s_zero = pg.s_zero; pd.n_pos = pg.n_pos;
         const int wpb = weighted ? kWarpsWeighted : kWarpsUnweighted;
         const int stride = weighted ? PosStage<kWarpsWeighted, 1, true>(pg.n_pos).stride
                                     : PosStage<kWarpsUnweighted, 2, false>(pg.n_pos).stride;
-        const int budgets[3] = {weighted ? 74 * 1024 : 112 * 1024, 112 * 1024, 224 * 1024};   // 3 / 2 / 1 blocks per SM
+        const int budgets[3] = {112 * 1024, 112 * 1024, 224 * 1024};                          // 2 / 2 / 1 blocks per SM
         pd.n_stages = 0;
         for (int b = 0; b < 3 && pd.n_stages < 2; ++b) pd.n_stages = std::min(kMaxStages, (budgets[b] - kPosHeader) / stride);
         if (const char *e = getenv("BSH_STAGES")) pd.n_stages = std::min(pd.n_stages, std::max(2, atoi(e)));

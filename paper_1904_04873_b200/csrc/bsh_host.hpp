@@ -106,7 +106,7 @@ struct PosGeometry {
     int off_table, s_max, n_pos, s_zero;
 };
 
-inline PosGeometry pos_geometry(const TableGeometry &tg, int n_bins, int n_f0, int NW)
+inline PosGeometry pos_geometry(const TableGeometry &tg, int n_bins, int n_f0, int NW, int tile_bins = 0)
 {
     PosGeometry g;
     if (tg.clamp) {
@@ -115,7 +115,7 @@ inline PosGeometry pos_geometry(const TableGeometry &tg, int n_bins, int n_f0, i
         g.n_pos = g.s_max + 1;
         g.s_zero = 0;
     } else {
-        const int tile = 32 * NW;
+        const int tile = tile_bins > 0 ? tile_bins : 32 * NW;
         const int w_min = n_f0 <= tile ? n_f0 : ((n_f0 % tile) ? (n_f0 % tile) : tile);
         g.off_table = 0;
         g.s_max = n_bins - w_min;

@@ -4,7 +4,7 @@
 // SFT) triple on extracting a 96-bit window at an arbitrary bit offset.  Here the window of EVERY start position is
 // precomputed once per patch (build_position_table_kernel: [N_pad][n_pos] entries of 16 bytes), streamed through shared
 // memory in stages of kStageSfts SFTs by 1-D TMA bulk copies, and read with one 16-byte shared-memory load at
-// row + position.  Blocks are 8 (unweighted) or 4 (weighted) full warps; warp w of a block works on pixel group
+// row + position.  Blocks are 8 full warps; warp w of a block works on pixel group
 // oct * WPB + w, so all warps share the staged table rows and the (cos, sin)(Omega_p t_i) rows, and the four SM
 // sub-partitions carry the same number of warps.  There is no block-wide barrier in the SFT loop: a stage is refilled by
 // whichever warp releases it last (shared-memory counter), and warps wait only on the stage's "full" mbarrier.
@@ -26,7 +26,7 @@ constexpr int kMaxStages = 6;
 constexpr int kPosHeader = 128;       // full[kMaxStages] mbarriers + done[kMaxStages] counters
 constexpr int kListCap = 64;          // deferred breaks per (thread, pixel); flushed when more than 32 are pending
 constexpr int kWarpsUnweighted = 8;   // warps per block = pixel groups per block
-constexpr int kWarpsWeighted = 4;
+constexpr int kWarpsWeighted = 8;     // (4-warp blocks, 3 per SM, measured 25.5 ms against 22.1 ms on config 2)
 
 // ---------------------------------------------------------------------------------------------------------------------
 // Position table: ptab[i][p] = window words of SFT i starting at slab column (p - off_table), zero outside [0, K) and
@@ -355,7 +355,7 @@ __device__ __forceinline__ void accumulate_bins(float (&acc)[NB], const Win<NW> 
 }
 
 template <int NW, int NB, bool CLAMP>
-__global__ void __launch_bounds__(32 * kWarpsWeighted, 3) stage1_weighted_pos_kernel(const PosParams p)
+__global__ void __launch_bounds__(32 * kWarpsWeighted, 2) stage1_weighted_pos_kernel(const PosParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int WPB = kWarpsWeighted;
