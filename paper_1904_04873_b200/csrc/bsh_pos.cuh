@@ -26,6 +26,10 @@ constexpr int kMaxStages = 6;
 constexpr int kPosHeader = 128;       // full[kMaxStages] mbarriers + done[kMaxStages] counters
 constexpr int kListCap = 64;          // deferred breaks per (thread, pixel); flushed when more than 32 are pending
 constexpr int kWarpsUnweighted = 8;   // warps per block = pixel groups per block
+#ifndef BSH_W_UNROLL
+#define BSH_W_UNROLL 16
+#endif
+constexpr int kWeightedUnroll = BSH_W_UNROLL;   // SFTs of a stage unrolled in the weighted kernel's inner loop
 constexpr int kWarpsWeighted = 8;     // (4-warp blocks, 3 per SM, measured 25.5 ms against 22.1 ms on config 2)
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -394,7 +398,7 @@ __global__ void __launch_bounds__(32 * kWarpsWeighted, 2) stage1_weighted_pos_ke
         const double2 *cs = reinterpret_cast<const double2 *>(sp + L.tab_bytes);
         const double *d = reinterpret_cast<const double *>(sp + L.tab_bytes + L.cs_bytes) + pc.warp;
         const float *wv = reinterpret_cast<const float *>(sp + L.tab_bytes + L.cs_bytes + L.d_bytes);
-#pragma unroll 2
+#pragma unroll(kWeightedUnroll)
         for (int k = 0; k < kStageSfts; ++k) {
             const double2 csk = cs[k];
             const double B = binary_term(tc, csk.x, csk.y);
