@@ -752,10 +752,25 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
     ctx->st.n_passes = pd.passes;
 
     CK(cudaEventRecord(ctx->ev[4], ctx->stream));
-    TRY(sort_candidates(ctx, (RawCand *)ctx->cand.p, n_cand));
+    RawCand *sorted = (RawCand *)ctx->cand.p;
+    if (n_cand > (unsigned)kSortTile && (uint64_t)n_cand > want && getenv("BSH_FULL_SORT") == nullptr) {
+        // only the candidates at or above the k-th largest key take part in the sort (ties at the cut included)
+        TRY(ensure(ctx, ctx->keys, (size_t)kCandCap * sizeof(RawCand)));
+        select_cut_kernel<<<1, 1024, 0, ctx->stream>>>((const RawCand *)ctx->cand.p, n_cand, (unsigned int)want,
+                                                       (RawCand *)ctx->keys.p, (unsigned int *)ctx->cand_count.p + 1);
+        count_launch(ctx);
+        CK(cudaMemcpyAsync(ctx->pinned_count + 1, (unsigned int *)ctx->cand_count.p + 1, sizeof(unsigned int),
+                           cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+        const unsigned int n_sel = ctx->pinned_count[1];
+        if (n_sel < want || n_sel > n_cand) return fail(ctx, BSH_ECUDA, "toplist pre-selection kept %u of %u", n_sel, n_cand);
+        sorted = (RawCand *)ctx->keys.p;
+        TRY(sort_candidates(ctx, sorted, n_sel));
+    } else {
+        TRY(sort_candidates(ctx, sorted, n_cand));
+    }
     const int n_keep = (int)want;
-    finalize_top_kernel<<<(pd.topk + 255) / 256, 256, 0, ctx->stream>>>((const RawCand *)ctx->cand.p, n_keep, pd.topk,
-                                                                      weighted ? 1 : 0, d_top);
+    finalize_top_kernel<<<(pd.topk + 255) / 256, 256, 0, ctx->stream>>>(sorted, n_keep, pd.topk, weighted ? 1 : 0, d_top);
     count_launch(ctx);
     {
         const TableCache &c = ctx->cache[pd.cache_slot];
@@ -764,7 +779,7 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
         bsh_grid g = {};
         g.n_pix = pd.n_pix; g.n_ap = pd.n_ap; g.n_P = pd.n_P; g.n_tasc = pd.n_tasc; g.n_f0 = pd.n_f0; g.k_band0 = pd.k_band0;
         const TrackTables t = make_track_tables(c, &s, &g, (const double *)ctx->dtab.p, pd.R);
-        rescore_kernel<<<(n_keep * 32 + 255) / 256, 256, 0, ctx->stream>>>(t, pd.d_peak, pd.words_per_row, pd.d_w,
+        rescore_kernel<<<n_keep, kCandThreads, 0, ctx->stream>>>(t, pd.d_peak, pd.words_per_row, pd.d_w,
                                                                           weighted ? 1 : 0, d_top, n_keep);
         count_launch(ctx);
     }
@@ -803,7 +818,7 @@ int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, c
     CK(cudaEventRecord(ctx->ev[6], ctx->stream));
     TRY(build_dtable(ctx, grid, c, 1, ctx->nvec2, ctx->dtab2));
     const TrackTables t = make_track_tables(c, sfts, grid, (const double *)ctx->dtab2.p, 1);
-    stage2_kernel<<<(unsigned)(((int64_t)n_cands * 32 + 255) / 256), 256, 0, ctx->stream>>>(t, d_rho, rho_row_stride,
+    stage2_kernel<<<(unsigned)n_cands, kCandThreads, 0, ctx->stream>>>(t, d_rho, rho_row_stride,
                                                                                           sfts->d_w, d_cands, n_cands);
     count_launch(ctx);
     CK(cudaGetLastError());

@@ -621,6 +621,72 @@ __device__ __forceinline__ bool cand_before(const RawCand &a, const RawCand &b)
     return a.key > b.key || (a.key == b.key && a.index < b.index);
 }
 
+// Pre-selection for the toplist (L217, L225): the k-th largest key of the n candidates is found by an MSB-first radix
+// select (4 passes of 8 bits, 256-bin shared-memory histogram), then every candidate with key >= that value is copied
+// to `out` (all ties AT the cut are kept, so the (key desc, index asc) order of R-11 is decided by the sort that
+// follows).  One block; n <= 2^20.  out_count[0] = number of candidates kept (>= k).
+__global__ void __launch_bounds__(1024) select_cut_kernel(const RawCand *__restrict__ cand, unsigned int n, unsigned int k,
+                                                          RawCand *__restrict__ out, unsigned int *__restrict__ out_count)
+{
+    __shared__ unsigned int hist[256];
+    __shared__ unsigned int s_prefix, s_k, s_n_out;
+    __shared__ unsigned int s_min[32], s_max[32];
+    // common leading bits of all keys need no pass (number counts of a patch differ in their low bits only, and a pass
+    // over identical digits would serialise every shared-memory atomic on one address)
+    unsigned int kmin = 0xFFFFFFFFu, kmax = 0u;
+    for (unsigned int i = threadIdx.x; i < n; i += blockDim.x) {
+        const unsigned int key = cand[i].key;
+        kmin = key < kmin ? key : kmin;
+        kmax = key > kmax ? key : kmax;
+    }
+    kmin = __reduce_min_sync(0xFFFFFFFFu, kmin);
+    kmax = __reduce_max_sync(0xFFFFFFFFu, kmax);
+    if ((threadIdx.x & 31) == 0) { s_min[threadIdx.x >> 5] = kmin; s_max[threadIdx.x >> 5] = kmax; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (unsigned int w = 1; w < (blockDim.x >> 5); ++w) {
+            kmin = s_min[w] < kmin ? s_min[w] : kmin;
+            kmax = s_max[w] > kmax ? s_max[w] : kmax;
+        }
+        const unsigned int diff = kmin ^ kmax;
+        const int top = diff ? 31 - __clz(diff) : -1;    // highest bit in which two keys differ
+        const int first_shift = top < 0 ? -8 : (top / 8) * 8;
+        s_prefix = first_shift + 8 >= 32 ? 0u : (kmax & (0xFFFFFFFFu << (first_shift + 8)));
+        s_k = k;
+        s_n_out = 0u;
+        s_min[0] = (unsigned int)(first_shift + 8);      // passes start below this bit
+    }
+    __syncthreads();
+    for (int shift = (int)s_min[0] - 8; shift >= 0; shift -= 8) {
+        for (unsigned int t = threadIdx.x; t < 256; t += blockDim.x) hist[t] = 0u;
+        __syncthreads();
+        const unsigned int prefix = s_prefix;
+        const unsigned int hi_mask = shift == 24 ? 0u : (0xFFFFFFFFu << (shift + 8));
+        for (unsigned int i = threadIdx.x; i < n; i += blockDim.x) {
+            const unsigned int key = cand[i].key;
+            if ((key & hi_mask) == prefix) atomicAdd(&hist[(key >> shift) & 255u], 1u);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned int need = s_k, d = 255u;
+            for (;; --d) {                               // digits above d hold fewer than `need` candidates
+                if (hist[d] >= need || d == 0u) break;
+                need -= hist[d];
+            }
+            s_k = need;
+            s_prefix = prefix | (d << shift);
+        }
+        __syncthreads();
+    }
+    const unsigned int cut = s_prefix;
+    for (unsigned int i = threadIdx.x; i < n; i += blockDim.x) {
+        const RawCand rc = cand[i];
+        if (rc.key >= cut) out[atomicAdd(&s_n_out, 1u)] = rc;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) out_count[0] = s_n_out;
+}
+
 __global__ void pad_candidates_kernel(RawCand *buf, unsigned int n, unsigned int n_pow2)
 {
     const unsigned int i = blockIdx.x * blockDim.x + threadIdx.x + n;
@@ -718,18 +784,24 @@ __device__ __forceinline__ int warp_sum_int(int v)
     return v;
 }
 
-__global__ void __launch_bounds__(256) rescore_kernel(const TrackTables t, const uint32_t *__restrict__ peak,
-                                                      int words_per_row, const float *__restrict__ w, int weighted_rank,
-                                                      bsh_cand *__restrict__ cands, int n_cands)
+// One block of kCandThreads threads per candidate: thread t takes SFTs t, t + kCandThreads, ... in order, then a fixed
+// xor-shuffle tree inside each warp and the warp partials in warp order (R-20: deterministic run to run).
+constexpr int kCandThreads = 128;
+
+__global__ void __launch_bounds__(kCandThreads) rescore_kernel(const TrackTables t, const uint32_t *__restrict__ peak,
+                                                               int words_per_row, const float *__restrict__ w,
+                                                               int weighted_rank, bsh_cand *__restrict__ cands, int n_cands)
 {
-    const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
+    __shared__ int sh_n[kCandThreads / 32];
+    __shared__ float sh_w[kCandThreads / 32];
+    const int c = blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (c >= n_cands) return;
     const TemplateCoord tc = decode_template(t, cands[c].index);
     const TemplateConst k = template_const(t, tc);
     int n = 0;
     float nw = 0.0f;
-    for (int i = lane; i < t.n_sft; i += 32) {
+    for (int i = threadIdx.x; i < t.n_sft; i += kCandThreads) {
         const int col = track_column(k, i, t.n_bins);
         if (col >= 0 && ((peak[(int64_t)i * words_per_row + (col >> 5)] >> (col & 31)) & 1u)) {
             n += 1;
@@ -738,7 +810,10 @@ __global__ void __launch_bounds__(256) rescore_kernel(const TrackTables t, const
     }
     n = warp_sum_int(n);
     nw = warp_sum(nw);
-    if (lane == 0) {
+    if (lane == 0) { sh_n[warp] = n; sh_w[warp] = nw; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < kCandThreads / 32; ++q) { n += sh_n[q]; nw += sh_w[q]; }
         if (weighted_rank) {
             cands[c].count = n;                  // wcount keeps the value that ranked the template
         } else {
@@ -747,17 +822,18 @@ __global__ void __launch_bounds__(256) rescore_kernel(const TrackTables t, const
     }
 }
 
-__global__ void __launch_bounds__(256) stage2_kernel(const TrackTables t, const float *__restrict__ rho, int64_t stride,
-                                                     const float *__restrict__ w, bsh_cand *__restrict__ cands,
-                                                     int n_cands)
+__global__ void __launch_bounds__(kCandThreads) stage2_kernel(const TrackTables t, const float *__restrict__ rho,
+                                                              int64_t stride, const float *__restrict__ w,
+                                                              bsh_cand *__restrict__ cands, int n_cands)
 {
-    const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
+    __shared__ float sh_p[kCandThreads / 32];
+    const int c = blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (c >= n_cands) return;
     const TemplateCoord tc = decode_template(t, cands[c].index);
     const TemplateConst k = template_const(t, tc);
     float pw = 0.0f;
-    for (int i = lane; i < t.n_sft; i += 32) {
+    for (int i = threadIdx.x; i < t.n_sft; i += kCandThreads) {
         const int col = track_column(k, i, t.n_bins);
         if (col >= 0) {
             const float r = rho[(int64_t)i * stride + col];
@@ -765,7 +841,10 @@ __global__ void __launch_bounds__(256) stage2_kernel(const TrackTables t, const 
         }
     }
     pw = warp_sum(pw);
-    if (lane == 0) {
+    if (lane == 0) sh_p[warp] = pw;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < kCandThreads / 32; ++q) pw += sh_p[q];
         cands[c].power = pw;
         cands[c].flags |= 2u;
     }
