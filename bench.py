@@ -35,7 +35,7 @@ UNIT = "accumulations/s"
 # --- roofline model of the stage-1 accumulation kernel -----------------------------------------
 # Unit of work: one (pixel, binary template, SFT) TRIPLE = n_f0 (90) accumulations.  The kernel is bound on chip by plain
 # instruction throughput: every pipe it uses (integer ALU, FP64, LSU/shared memory) is 40-60 % busy and the warp
-# schedulers issue 63 % of their slots (ncu, profiles/r01c_stage1_pix_full.md); HBM is idle.  Roofline = warp-issue peak.
+# schedulers issue 63 % of their slots (ncu, profiles/r01d_stage1_pix_full.md); HBM is idle.  Roofline = warp-issue peak.
 N_SM = 148
 LANES_PER_SM_CLK = 128            # 4 SMSPs x 32 lanes: one warp instruction per scheduler per clock
 # algorithmic lane-instructions per triple -- what this formulation must execute whatever the schedule:
@@ -54,8 +54,8 @@ ALU_OPS_PER_TRIPLE = 6.0 + 1.125 + 3.0
 OPS_PER_TRIPLE_WEIGHTED_FIXED = 19.0
 OPS_PER_ACC_WEIGHTED = 2.0
 GATHER_LANES_PER_SM_CLK = 32      # north_star bound (b) read literally: one 4-byte lane-gather per accumulation
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the kernel (ncu --set full, profiles/r01c_stage1_pix_full.md)
-NCU_DRAM_BYTES_PER_LAUNCH = 12731648 + 747520
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the kernel (ncu --set full, profiles/r01d_stage1_pix_full.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 12775424 + 674304
 
 
 def measured_peaks():
