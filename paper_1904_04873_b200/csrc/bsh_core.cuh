@@ -429,6 +429,87 @@ BSH_HD int32_t count_at(const Counter<NW, HP> &c, int w, int b)
     return n;
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// Lean resolution of deferred breaks (used by the pixel-lane kernel, bsh_pix.cuh; __host__ __device__ so that the host
+// emulation test runs the same code).
+// ---------------------------------------------------------------------------------------------------------------------
+BSH_HD float fast_divide(float a, float b)
+{
+#ifdef __CUDA_ARCH__
+    return __fdividef(a, b);
+#else
+    return a / b;
+#endif
+}
+
+// Exact window of a (pixel, template, SFT) whose rounded shift is not the same at both ends of the f0 tile (R-7).
+// One break (|sL - s0| == 1): r_j is monotone in j, so there is one bin jb with shift(jb - 1) == s0, shift(jb) == sL.
+// jb is estimated from the distance of fl(u0 g) + 1/2 to the integer it crosses (FP32 division) and then corrected on
+// the canonical evaluation itself -- the estimate only saves work, the result is exact.  More breaks (unphysical
+// |g| n_f) or clamped positions: the generic per-bin routine of bsh_core.cuh.
+template <int NW, bool CLAMP>
+BSH_HD Win<NW> exact_window_pos(const TrackConst &tc, const uint4 *row_positions, double D, double B)
+{
+    const double g = dsub(D, B);
+    const double t0 = dadd(dmul(tc.u0, g), 0.5);
+    const int32_t s0 = floor_plus(t0, tc.magic, tc.off);
+    const int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
+    const int32_t d = sL - s0;
+    if (CLAMP || (d != 1 && d != -1)) return track_window_pos<NW, CLAMP>(tc, row_positions, D, B);
+    const double fl0 = floor(t0);
+    const float dist = (float)((d > 0 ? fl0 + 1.0 : fl0) - t0);       // signed distance to the crossed integer
+    int j = (int)ceilf(fast_divide(dist, (float)g));
+    j = j < 1 ? 1 : (j > tc.n_fj - 1 ? tc.n_fj - 1 : j);
+    while (j > 1 && shift_of(dadd(tc.u0, (double)(j - 1)), g, tc.magic, tc.off) != s0) --j;
+    while (j < tc.n_fj - 1 && shift_of(dadd(tc.u0, (double)j), g, tc.magic, tc.off) == s0) ++j;
+    const Win<NW> a = load_position<NW>(row_positions, s0);
+    const Win<NW> b = load_position<NW>(row_positions, sL);
+    Win<NW> out;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+        const int rel = j - 32 * w;                      // bins >= j take the second window
+        const uint32_t m = rel <= 0 ? 0xFFFFFFFFu : (rel >= 32 ? 0u : (0xFFFFFFFFu << rel));
+        out.x[w] = (a.x[w] & ~m) | (b.x[w] & m);
+    }
+    return out;
+}
+
+// The deferred windows of one flush are first summed in a small bit-sliced accumulator (kFixPlanes planes, ripple
+// carry: 2 kFixPlanes LOP per word and window instead of 2 (5 + HP)), which is then added to the counter once.
+constexpr int kFixPlanes = 7;                            // up to 127 windows per flush (kListCap = 64)
+
+template <int NW>
+BSH_HD void fix_accumulate(uint32_t (&tp)[kFixPlanes][NW], const Win<NW> &x)
+{
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+        uint32_t carry = x.x[w];
+#pragma unroll
+        for (int q = 0; q < kFixPlanes; ++q) {
+            const uint32_t t = tp[q][w] & carry;
+            tp[q][w] ^= carry;
+            carry = t;
+        }
+    }
+}
+
+template <int NW, int HP>
+BSH_HD void fix_merge(Counter<NW, HP> &c, const uint32_t (&tp)[kFixPlanes][NW])
+{
+    static_assert(kLowPlanes + HP >= kFixPlanes, "counter narrower than the fix-up accumulator");
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+        uint32_t carry = 0u;
+#pragma unroll
+        for (int q = 0; q < kLowPlanes + HP; ++q) {
+            uint32_t &pl = q < kLowPlanes ? c.low[q < kLowPlanes ? q : 0][w] : c.hi[q < kLowPlanes ? 0 : q - kLowPlanes][w];
+            const uint32_t a = pl, b = q < kFixPlanes ? tp[q < kFixPlanes ? q : 0][w] : 0u;
+            pl = xor3(a, b, carry);
+            carry = maj3(a, b, carry);
+        }
+    }
+}
+
 BSH_HD uint32_t valid_mask(int n_fj, int w)
 {
     const int rel = n_fj - 32 * w;

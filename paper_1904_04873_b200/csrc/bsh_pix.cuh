@@ -171,74 +171,6 @@ __device__ __forceinline__ Win<NW> pix_load(const unsigned char *tab, int n_pos,
     return w;
 }
 
-// Exact window of a (pixel, template, SFT) whose rounded shift is not the same at both ends of the f0 tile (R-7).
-// One break (|sL - s0| == 1): r_j is monotone in j, so there is one bin jb with shift(jb - 1) == s0, shift(jb) == sL.
-// jb is estimated from the distance of fl(u0 g) + 1/2 to the integer it crosses (FP32 division) and then corrected on
-// the canonical evaluation itself -- the estimate only saves work, the result is exact.  More breaks (unphysical
-// |g| n_f) or clamped positions: the generic per-bin routine of bsh_core.cuh.
-template <int NW, bool CLAMP>
-__device__ __forceinline__ Win<NW> pix_exact_window(const TrackConst &tc, const uint4 *row_positions, double D, double B)
-{
-    const double g = __dsub_rn(D, B);
-    const double t0 = __dadd_rn(__dmul_rn(tc.u0, g), 0.5);
-    const int32_t s0 = floor_plus(t0, tc.magic, tc.off);
-    const int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
-    const int32_t d = sL - s0;
-    if (CLAMP || (d != 1 && d != -1)) return track_window_pos<NW, CLAMP>(tc, row_positions, D, B);
-    const double fl0 = floor(t0);
-    const float dist = (float)((d > 0 ? fl0 + 1.0 : fl0) - t0);       // signed distance to the crossed integer
-    int j = (int)ceilf(__fdividef(dist, (float)g));
-    j = j < 1 ? 1 : (j > tc.n_fj - 1 ? tc.n_fj - 1 : j);
-    while (j > 1 && shift_of(__dadd_rn(tc.u0, (double)(j - 1)), g, tc.magic, tc.off) != s0) --j;
-    while (j < tc.n_fj - 1 && shift_of(__dadd_rn(tc.u0, (double)j), g, tc.magic, tc.off) == s0) ++j;
-    const Win<NW> a = load_position<NW>(row_positions, s0);
-    const Win<NW> b = load_position<NW>(row_positions, sL);
-    Win<NW> out;
-#pragma unroll
-    for (int w = 0; w < NW; ++w) {
-        const int rel = j - 32 * w;                      // bins >= j take the second window
-        const uint32_t m = rel <= 0 ? 0xFFFFFFFFu : (rel >= 32 ? 0u : (0xFFFFFFFFu << rel));
-        out.x[w] = (a.x[w] & ~m) | (b.x[w] & m);
-    }
-    return out;
-}
-
-// The deferred windows of one flush are first summed in a small bit-sliced accumulator (kFixPlanes planes, ripple
-// carry: 2 kFixPlanes LOP per word and window instead of 2 (5 + HP)), which is then added to the counter once.
-constexpr int kFixPlanes = 7;                            // up to 127 windows per flush (kListCap = 64)
-
-template <int NW>
-__device__ __forceinline__ void fix_accumulate(uint32_t (&tp)[kFixPlanes][NW], const Win<NW> &x)
-{
-#pragma unroll
-    for (int w = 0; w < NW; ++w) {
-        uint32_t carry = x.x[w];
-#pragma unroll
-        for (int q = 0; q < kFixPlanes; ++q) {
-            const uint32_t t = tp[q][w] & carry;
-            tp[q][w] ^= carry;
-            carry = t;
-        }
-    }
-}
-
-template <int NW, int HP>
-__device__ __forceinline__ void fix_merge(Counter<NW, HP> &c, const uint32_t (&tp)[kFixPlanes][NW])
-{
-    static_assert(kLowPlanes + HP >= kFixPlanes, "counter narrower than the fix-up accumulator");
-#pragma unroll
-    for (int w = 0; w < NW; ++w) {
-        uint32_t carry = 0u;
-#pragma unroll
-        for (int q = 0; q < kLowPlanes + HP; ++q) {
-            uint32_t &pl = q < kLowPlanes ? c.low[q < kLowPlanes ? q : 0][w] : c.hi[q < kLowPlanes ? 0 : q - kLowPlanes][w];
-            const uint32_t a = pl, b = q < kFixPlanes ? tp[q < kFixPlanes ? q : 0][w] : 0u;
-            pl = xor3(a, b, carry);
-            carry = maj3(a, b, carry);
-        }
-    }
-}
-
 // One SFT (slot K of the unrolled block of 32) for both templates of the thread.
 template <int K, int NW, int HP, bool CLAMP>
 __device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char *tab, int n_pos, const double2 *bpair,
@@ -407,7 +339,7 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
                     const double2 c = p.cs[(int64_t)ip * p.n_pad + i];
                     const double B = binary_term(tc, c.x, c.y);
                     const double D = p.dpix[((((int64_t)pg * (p.n_pad >> 1)) + (i >> 1)) * 32 + lane) * 2 + (i & 1)];
-                    fix_accumulate<NW>(tp, pix_exact_window<NW, CLAMP>(tc, p.ptab + (int64_t)i * p.n_pos, D, B));
+                    fix_accumulate<NW>(tp, exact_window_pos<NW, CLAMP>(tc, p.ptab + (int64_t)i * p.n_pos, D, B));
                 }
                 fix_merge<NW, HP>(cnt[r], tp);
                 npend[r] = 0;

@@ -24,7 +24,7 @@ def emu():
     return C.CDLL(lib)
 
 
-def run_emu(emu, wl, peak, weighted=False, force_clamp=False, nw=0):
+def run_emu(emu, wl, peak, weighted=False, force_clamp=False, nw=0, pix=False):
     f64 = lambda a: np.ascontiguousarray(a, np.float64)
     arrs = [f64(wl.t_mid), f64(wl.v_over_c), f64(wl.alpha), f64(wl.delta), f64(wl.ap), f64(wl.P), f64(wl.tasc_frac)]
     t_mid, v, alpha, delta, ap, P, tf = arrs
@@ -37,7 +37,7 @@ def run_emu(emu, wl, peak, weighted=False, force_clamp=False, nw=0):
     rc = emu.emu_stage1(C.c_int(wl.n_sft), p(t_mid), p(v), C.c_double(wl.t_search_mid), C.c_int64(wl.k_slab0),
                         C.c_int(wl.n_bins), C.c_int64(wl.k_band0), C.c_int(wl.n_f0), C.c_int(wl.n_pix), p(alpha), p(delta),
                         C.c_int(len(ap)), p(ap), C.c_int(len(P)), p(P), C.c_int(len(tf)), p(tf), p(peak),
-                        C.c_int(peak.shape[1]), p(w), C.c_int(int(weighted)), C.c_int(int(force_clamp)), C.c_int(nw),
+                        C.c_int(peak.shape[1]), p(w), C.c_int(2 if pix else int(weighted)), C.c_int(int(force_clamp)), C.c_int(nw),
                         p(counts), p(wcounts), p(info))
     assert rc == 0
     return counts, wcounts, info
@@ -50,6 +50,8 @@ def test_emulated_kernel_logic_matches_oracle_config1(emu, pixel, force_clamp, n
     pk = oracle.peakgram(wl.rho)
     want, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
     got, _, info = run_emu(emu, wl, pk, force_clamp=force_clamp, nw=nw)
+    got_pix, _, _ = run_emu(emu, wl, pk, force_clamp=force_clamp, nw=nw, pix=True)
+    assert np.array_equal(got_pix, want)
     if pixel == "ecliptic":
         assert info[0] == 1, "tracks leave the slab here: the clamped table must be chosen"
     assert np.array_equal(got, want)
@@ -67,6 +69,8 @@ def test_emulated_kernel_logic_ragged_sizes_and_breaks(emu, n_sft, n_f0, margin,
     for force_clamp in (False, True):
         got, _, info = run_emu(emu, wl, pk, force_clamp=force_clamp)
         assert np.array_equal(got, want), (force_clamp, info)
+        got, _, info = run_emu(emu, wl, pk, force_clamp=force_clamp, pix=True)      # position table + lean fix-ups
+        assert np.array_equal(got, want), ("pix", force_clamp, info)
         _, got_w, _ = run_emu(emu, wl, pk, weighted=True, force_clamp=force_clamp)
         assert np.allclose(got_w, want_w, rtol=1e-5, atol=1e-6)
 
@@ -81,4 +85,19 @@ def test_emulated_kernel_logic_multiple_breaks_per_band(emu):
     got, _, info = run_emu(emu, wl, pk)
     assert info[0] == 1
     assert np.array_equal(got, want)
+    got, _, _ = run_emu(emu, wl, pk, pix=True)
+    assert np.array_equal(got, want)
     assert want.max() > 0
+
+
+def test_emulated_pixel_lane_fixups_with_many_breaks(emu):
+    """A wide band (n_f0 = 96) at a high frequency with fast orbits: about 1 % of the 32000 (pixel, template, SFT) triples
+    break inside the tile (345, in both directions), so the estimated break bin of exact_window_pos() is exercised all
+    over the tile."""
+    wl = synth.noise_workload(seed=91, n_sft=400, n_f0=96, margin=250, f_band_start=900.0, n_pix_side=2,
+                              ap=(30.0, 40.0), P_days=(15.0, 16.0), n_t=5)
+    pk = oracle.peakgram(wl.rho)
+    want, _ = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL, want_wcount=False)
+    got, _, info = run_emu(emu, wl, pk, pix=True)
+    assert info[0] == 0, "unclamped geometry expected"
+    assert np.array_equal(got, want)
