@@ -39,12 +39,12 @@ UNIT = "accumulations/s"
 N_SM = 148
 LANES_PER_SM_CLK = 128            # 4 SMSPs x 32 lanes: one warp instruction per scheduler per clock
 # algorithmic lane-instructions per triple -- what this formulation must execute whatever the schedule:
-#   FP64  g = D - B (1), y at both band ends (2), + 1/2 (2), floor by magic add (2), equal-shift test (1)           8
+#   FP64  g = D - B (1), y at both band ends (2), round by magic add (2), equal-shift test (1)                      6
 #   count 3 window words x full adder (2 LOP3) + ripple into the 6 high planes once per 32 SFTs (36 / 32)           7.125
 #   INT   position select on a break (1), break mask (1), shared-memory address (1)                                 3
 #   LSU   window read (LDS.64 + LDS.32) 2, binary terms of 2 templates per load 0.5, Doppler terms of 2 SFTs
 #         per load shared by 2 templates 0.25                                                                       2.75
-ALGO_OPS_PER_TRIPLE = 8.0 + 7.125 + 3.0 + 2.75
+ALGO_OPS_PER_TRIPLE = 6.0 + 7.125 + 3.0 + 2.75
 # secondary views: the shared-memory data pipe (one 128-byte wavefront per clock per SM) and the integer-ALU pipe alone
 SMEM_BYTES_PER_CLK_SM = 128
 SMEM_BYTES_PER_TRIPLE = 12.0 + 4.0 + 4.0      # 96-bit window + D (8 B per 2 templates) + B (one wavefront per 32 triples)

@@ -80,7 +80,8 @@ void orc_peakgram(const float *rho, int32_t n_sft, int32_t n_bins, float rho_th,
 }
 
 /* ---------------------------------------------------------------------------------------------------------
- * Track, DIRECT mode: Eq. (15) as printed, then bin = round((f - f_slab_start) * T)   (R-1: floor(x + 1/2)).
+ * Track, DIRECT mode: Eq. (15) as printed, then bin = round((f - f_slab_start) * T)   (R-1: to the nearest integer,
+ * ties to even -- IEEE-754 round-to-nearest, nearbyint() in the default rounding mode).
  * Returns the slab column (may lie outside [0, K): such an SFT contributes nothing, R-6).
  * If x_out != NULL it receives x, the unrounded bin coordinate (for near-tie flagging).
  * ------------------------------------------------------------------------------------------------------- */
@@ -100,7 +101,7 @@ int64_t orc_track_direct(const orc_problem *pb, int pix, int ia, int ip, int it,
     const double f_slab = (double)pb->k_slab0 / T;
     const double x = (f - f_slab) * T;
     if (x_out) *x_out = x;
-    return (int64_t)floor(x + 0.5);
+    return (int64_t)nearbyint(x);
 }
 
 /* ---------------------------------------------------------------------------------------------------------
@@ -137,8 +138,7 @@ static int64_t canon_bin(const orc_problem *pb, double D, double A, double C, do
     const double u = (double)(pb->k_band0 + j);
     const double y = u * g;
     if (y_out) *y_out = y;
-    const double t = y + 0.5;
-    const int64_t r = (int64_t)floor(t);
+    const int64_t r = (int64_t)nearbyint(y);             /* R-1: nearest integer, ties to even */
     return (pb->k_band0 - pb->k_slab0) + j + r;
 }
 

@@ -4,7 +4,7 @@
 // exercised by the host-side emulation test (tests/hostemu) without a GPU.  Nothing here is shared with oracle/.
 //
 // PAPER.md L102 Eq. (15): f(t) = f0 [1 + v.n/c - a_p Omega cos(Omega (t - t_asc))]; the slab column of template j at
-// SFT i is  k = m + j + r,  r = floor(fl(y + 1/2)),  y = fl(u_j g),  u_j = k_band0 + j,  g = fl(D - fl(A cphi)),
+// SFT i is  k = m + j + r,  r = round(y) (nearest, ties to even),  y = fl(u_j g),  u_j = k_band0 + j,  g = fl(D - fl(A cphi)),
 // cphi = fl(fl(C CA) + fl(S SA))  (R-5).  All FP64 operations are individually rounded (no FMA).
 #pragma once
 #include <stdint.h>
@@ -21,7 +21,7 @@ struct uint4 { uint32_t x, y, z, w; };
 
 namespace bsh {
 
-constexpr double kMagic = 6755399441055744.0;   // 1.5 * 2^52: fl_down(t + kMagic) carries floor(t) in its low word
+constexpr double kMagic = 6755399441055744.0;   // 1.5 * 2^52: fl(y + kMagic) carries round-to-nearest-even(y) in its low word
 constexpr int kMaxWords = 3;                    // f0 bins per pass <= 96 (three 32-bit window words)
 constexpr int kLowPlanes = 5;                   // carry-save levels = log2(SFTs per unrolled block)
 constexpr int kBlock = 32;                      // SFTs per unrolled block
@@ -51,22 +51,22 @@ BSH_HD double dsub(double a, double b)
 #endif
 }
 
-// off + floor(t) for |t| < 2^31, off an integer folded into `magic` = kMagic + off.
-BSH_HD int32_t floor_plus(double t, double magic, int32_t off)
+// r = y rounded to the nearest integer, ties to even (IEEE-754 default rounding; R-1), |y| < 2^31: the
+// low word of fl(y + 1.5 2^52) on the device (one FP64 add), nearbyint() on the host.
+BSH_HD int32_t round_int(double y)
 {
 #ifdef __CUDA_ARCH__
-    (void)off;
-    return __double2loint(__dadd_rd(t, magic));
+    return __double2loint(__dadd_rn(y, kMagic));
 #else
-    (void)magic;
-    return off + (int32_t)floor(t);
+    return (int32_t)nearbyint(y);
 #endif
 }
 
-// s = off + floor(fl(fl(u g) + 1/2))
+// s = off + round(fl(u g))   (`magic` is unused: kept so that the call sites read as before)
 BSH_HD int32_t shift_of(double u, double g, double magic, int32_t off)
 {
-    return floor_plus(dadd(dmul(u, g), 0.5), magic, off);
+    (void)magic;
+    return off + round_int(dmul(u, g));
 }
 
 BSH_HD uint32_t funnel_r(uint32_t lo, uint32_t hi, int sh)   // low 32 bits of ((hi:lo) >> (sh & 31))
@@ -444,20 +444,20 @@ BSH_HD float fast_divide(float a, float b)
 
 // Exact window of a (pixel, template, SFT) whose rounded shift is not the same at both ends of the f0 tile (R-7).
 // One break (|sL - s0| == 1): r_j is monotone in j, so there is one bin jb with shift(jb - 1) == s0, shift(jb) == sL.
-// jb is estimated from the distance of fl(u0 g) + 1/2 to the integer it crosses (FP32 division) and then corrected on
+// jb is estimated from the distance of fl(u0 g) to the half-integer it crosses (FP32 division) and then corrected on
 // the canonical evaluation itself -- the estimate only saves work, the result is exact.  More breaks (unphysical
 // |g| n_f) or clamped positions: the generic per-bin routine of bsh_core.cuh.
 template <int NW, bool CLAMP>
 BSH_HD Win<NW> exact_window_pos(const TrackConst &tc, const uint4 *row_positions, double D, double B)
 {
     const double g = dsub(D, B);
-    const double t0 = dadd(dmul(tc.u0, g), 0.5);
-    const int32_t s0 = floor_plus(t0, tc.magic, tc.off);
+    const double y0 = dmul(tc.u0, g);
+    const int32_t r0 = round_int(y0);
+    const int32_t s0 = tc.off + r0;
     const int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
     const int32_t d = sL - s0;
     if (CLAMP || (d != 1 && d != -1)) return track_window_pos<NW, CLAMP>(tc, row_positions, D, B);
-    const double fl0 = floor(t0);
-    const float dist = (float)((d > 0 ? fl0 + 1.0 : fl0) - t0);       // signed distance to the crossed integer
+    const float dist = (float)(((double)r0 + (d > 0 ? 0.5 : -0.5)) - y0);     // signed distance to the crossed half-integer
     int j = (int)ceilf(fast_divide(dist, (float)g));
     j = j < 1 ? 1 : (j > tc.n_fj - 1 ? tc.n_fj - 1 : j);
     while (j > 1 && shift_of(dadd(tc.u0, (double)(j - 1)), g, tc.magic, tc.off) != s0) --j;

@@ -134,22 +134,22 @@ __device__ __forceinline__ void pix_release(const PixParams &p, const PixStage &
 
 // Per-thread constants of the hot loop (the binary-term constants live in shared memory, only the fix-ups need them).
 struct PixConst {
-    double u0, uL, magic;
-    int32_t s_max, s_zero;
+    double u0, uL;
+    int32_t off, s_max, s_zero;
 };
 
 // Position (table entry) to read for one (pixel, template, SFT) and the break flag (R-7): the all-zero position on a
-// break.  Unclamped geometry: the two magic-add results are compared as doubles (equal doubles <=> equal low words),
+// break.  Unclamped geometry: the two magic-add results are compared as doubles (equal doubles <=> equal roundings),
 // which keeps the comparison on the FP64 pipe.
 template <bool CLAMP>
 __device__ __forceinline__ int32_t pix_position(const PixConst &k, double D, double B, bool &brk)
 {
     const double g = __dsub_rn(D, B);
-    const double m0 = __dadd_rd(__dadd_rn(__dmul_rn(k.u0, g), 0.5), k.magic);
-    const double mL = __dadd_rd(__dadd_rn(__dmul_rn(k.uL, g), 0.5), k.magic);
-    int32_t s0 = __double2loint(m0);
+    const double m0 = __dadd_rn(__dmul_rn(k.u0, g), kMagic);         // low word = round(fl(u0 g)), R-1
+    const double mL = __dadd_rn(__dmul_rn(k.uL, g), kMagic);
+    int32_t s0 = k.off + __double2loint(m0);
     if (CLAMP) {
-        int32_t sL = __double2loint(mL);
+        int32_t sL = k.off + __double2loint(mL);
         s0 = clamp_s(s0, k.s_max);
         sL = clamp_s(sL, k.s_max);                       // equal after clamping => every bin reads 0
         brk = s0 != sL;
@@ -187,8 +187,8 @@ __device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char 
         if (!CLAMP) {
             // one predicate from the FP64 compare drives both the mask update (predicated OR) and the position select
             const double g = __dsub_rn(D, Bv[r]);
-            const double m0 = __dadd_rd(__dadd_rn(__dmul_rn(k.u0, g), 0.5), k.magic);
-            const double mL = __dadd_rd(__dadd_rn(__dmul_rn(k.uL, g), 0.5), k.magic);
+            const double m0 = __dadd_rn(__dmul_rn(k.u0, g), kMagic);  // low word = round(fl(u0 g)) (R-1)
+            const double mL = __dadd_rn(__dmul_rn(k.uL, g), kMagic);
             asm("{\n\t"
                 ".reg .pred p;\n\t"
                 "setp.neu.f64 p, %2, %3;\n\t"
@@ -196,7 +196,8 @@ __device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char 
                 "selp.b32 %1, %5, %6, p;\n\t"
                 "}"
                 : "+r"(brk[r]), "=r"(s)
-                : "d"(m0), "d"(mL), "n"(1u << K), "r"(k.s_zero), "r"(__double2loint(m0)));
+                : "d"(m0), "d"(mL), "n"(1u << K), "r"(k.s_zero - k.off), "r"(__double2loint(m0)));
+            s += k.off;                                  // merges with the row offset below: one uniform add
         } else {
             bool b;
             s = pix_position<CLAMP>(k, D, Bv[r], b);
@@ -270,7 +271,7 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
     PixConst kc;
     kc.u0 = p.u0;
     kc.uL = p.u0 + (double)(p.n_fj - 1);
-    kc.magic = kMagic + (double)p.off;
+    kc.off = p.off;
     kc.s_max = p.s_max;
     kc.s_zero = p.s_zero;
 
@@ -326,7 +327,7 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
 #pragma unroll
             for (int r = 0; r < kPixTpl; ++r) {
                 TrackConst tc;
-                tc.u0 = kc.u0; tc.uL = kc.uL; tc.magic = kc.magic; tc.off = p.off; tc.s_max = p.s_max; tc.s_zero = p.s_zero;
+                tc.u0 = kc.u0; tc.uL = kc.uL; tc.magic = kMagic; tc.off = p.off; tc.s_max = p.s_max; tc.s_zero = p.s_zero;
                 tc.n_fj = p.n_fj;
                 tc.A = tcst[r * 4 + 0]; tc.CA = tcst[r * 4 + 1]; tc.SA = tcst[r * 4 + 2];
                 uint32_t tp[kFixPlanes][NW];

@@ -353,3 +353,23 @@ def noise_workload(seed: int, n_sft: int, n_f0: int, margin: int, f_band_start: 
     alpha, delta = patch_pixels(a0, d0, pixel_size(t_sft, f_band_start, 1.0), n_pix_side, n_pix_side)
     return _finish(f"noise-{seed}", seed, t_sft, starts, v, f_band_start, n_f0 / t_sft, margin, rho, w, alpha, delta,
                    np.asarray(ap, np.float64), np.asarray(P_days, np.float64) * DAY, tasc_fractions(n_t), topk)
+
+
+def tie_workload() -> Workload:
+    """Inputs whose bin coordinate y = u_j g lands EXACTLY on half-integers at j = 0 (R-1 pins the tie rule):
+    k_band0 = 2^17, one pixel at alpha = delta = 0 (n = (1, 0, 0) exactly), a_p = 0 (no binary term), and detector
+    velocities v_x / c = q 2^-18 for q = 1, 3, 5, -1, -3, 2, 0, 7, so that y = q / 2 at j = 0.  Powers alternate between
+    a peak on the even slab columns and none on the odd ones: a bin that is off by one changes the count."""
+    q = np.array([1, 3, 5, -1, -3, 2, 0, 7], np.float64)
+    n, t_sft, margin, n_f0 = len(q), 900.0, 8, 4
+    v = np.zeros((n, 3), np.float64)
+    v[:, 0] = q * 2.0 ** -18
+    starts = np.arange(n, dtype=np.float64) * 1800.0
+    rho = np.where(np.arange(n_f0 + 2 * margin)[None, :] % 2 == 0, 2.0, 0.5).astype(np.float32).repeat(n, axis=0)
+    k_band0 = 1 << 17
+    t_mid = starts + 0.5 * t_sft
+    return Workload(name="ties", seed=0, t_sft=t_sft, t_mid=t_mid, v_over_c=v,
+                    t_search_mid=0.5 * (starts[0] + starts[-1] + t_sft), k_slab0=k_band0 - margin,
+                    n_bins=n_f0 + 2 * margin, k_band0=k_band0, n_f0=n_f0, rho=np.ascontiguousarray(rho),
+                    w=np.ones(n, np.float32), alpha=np.zeros(1), delta=np.zeros(1), ap=np.zeros(1),
+                    P=np.array([15.0 * DAY]), tasc_frac=np.zeros(1), topk=4)

@@ -425,3 +425,21 @@ def test_search_patch_host_end_to_end(bsh, torch, ctx):
     assert np.all(np.diff(recs["power"]) <= 0)
     st = ctx.stats()
     assert st["launches"] > 0 and st["n_templates"] == 1620
+
+
+def test_ties_round_to_even_on_the_gpu(bsh, torch, ctx, monkeypatch):
+    """R-1: exact half-integer bin coordinates (synth.tie_workload): every kernel family rounds them like the oracle."""
+    wl = synth.tie_workload()
+    pk = oracle.peakgram(wl.rho)
+    want_n, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
+    for env in ({}, {"BSH_FORCE_PIX": "1"}, {"BSH_LEGACY": "1"}, {"BSH_FORCE_CLAMP": "1"}):
+        for key in ("BSH_FORCE_PIX", "BSH_LEGACY", "BSH_FORCE_CLAMP"):
+            monkeypatch.delenv(key, raising=False)
+        for key, val in env.items():
+            monkeypatch.setenv(key, val)
+        r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
+        assert np.array_equal(r["counts"], want_n), env
+        r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED)
+        assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=0), env
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED | bsh.BSH_NAIVE)
+    assert np.array_equal(r["counts"], want_n)

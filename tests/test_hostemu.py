@@ -101,3 +101,14 @@ def test_emulated_pixel_lane_fixups_with_many_breaks(emu):
     got, _, info = run_emu(emu, wl, pk, pix=True)
     assert info[0] == 0, "unclamped geometry expected"
     assert np.array_equal(got, want)
+
+
+def test_emulated_kernels_round_ties_to_even(emu):
+    """R-1 on the kernel side: exact half-integer bin coordinates (synth.tie_workload) give the oracle's counts."""
+    wl = synth.tie_workload()
+    pk = oracle.peakgram(wl.rho)
+    want, _ = oracle.stage1(wl, pk, None, mode=oracle.CANONICAL)
+    for pix in (False, True):
+        for force_clamp in (False, True):
+            got, _, _ = run_emu(emu, wl, pk, force_clamp=force_clamp, pix=pix)
+            assert np.array_equal(got, want), (pix, force_clamp)

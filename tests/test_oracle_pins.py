@@ -400,3 +400,26 @@ def test_injected_signal_is_loudest_and_count_matches_marcum_q():
     pw = oracle.stage2(wl, top, rho, None)
     assert int(top[np.argmax(pw)]) == want
     assert abs(pw[0] - n_sft * 1.3) < 5 * math.sqrt(n_sft * (1 + 2 * 0.3))     # E[rho] = 1 + |A|^2, var = 1 + 2|A|^2
+
+
+def test_ties_round_to_even():
+    """R-1: the bin is round(y) to the nearest integer, ties to even.  With the tie workload y = q / 2 exactly at j = 0
+    (k_band0 = 2^17, v_x / c = q 2^-18, n = (1, 0, 0), no binary term), so the expected bins follow from Python's own
+    round() (banker's rounding) -- nothing of the oracle is used to form them."""
+    wl = synth.tie_workload()
+    q = [1, 3, 5, -1, -3, 2, 0, 7]
+    want = np.array([wl.margin + round(v / 2) for v in q])
+    assert [round(v / 2) for v in q] == [0, 2, 2, 0, -2, 1, 0, 4]
+    assert np.array_equal(oracle.track(wl, 0, 0, 0, 0, 0, mode=oracle.CANONICAL), want)
+    # DIRECT evaluates Eq. (15) as printed: its x carries a few ulps of rounding, so at an exact tie it may fall on either
+    # side (these are the flagged near-ties of compare_modes); away from ties it must agree
+    direct = oracle.track(wl, 0, 0, 0, 0, 0, mode=oracle.DIRECT)
+    tie = np.array([v % 2 != 0 for v in q])
+    assert np.array_equal(direct[~tie], want[~tie]) and np.all(np.abs(direct[tie] - want[tie]) <= 1)
+    # one bin up the lattice (u = 2^17 + 1) y is no longer a tie: ordinary rounding of q/2 (1 + 2^-17)
+    want1 = np.array([wl.margin + 1 + math.floor(v / 2 * (1 + 2.0 ** -17) + 0.5) for v in q])
+    assert np.array_equal(oracle.track(wl, 0, 0, 0, 0, 1, mode=oracle.CANONICAL), want1)
+    # and the counts see the parity of the bins (peaks on even columns only)
+    pk = oracle.peakgram(wl.rho)
+    cnt, _ = oracle.stage1(wl, pk, None, mode=oracle.CANONICAL)
+    assert cnt[0] == int(np.sum(want % 2 == 0))
