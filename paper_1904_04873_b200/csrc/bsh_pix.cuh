@@ -159,15 +159,16 @@ __device__ __forceinline__ int32_t pix_position(const PixConst &k, double D, dou
     return brk ? k.s_zero : s0;
 }
 
-// Window of position s of stage row kk: words 0, 1 from the pair array, word 2 from the word array.
+// Window of table index idx = stage row kk * n_pos + position: words 0, 1 from the pair array, word 2 from the word
+// array.
 template <int NW>
-__device__ __forceinline__ Win<NW> pix_load(const unsigned char *tab, int n_pos, int kk, int32_t s)
+__device__ __forceinline__ Win<NW> pix_load(const unsigned char *tab, int n_pos, int32_t idx)
 {
     Win<NW> w;
-    const uint2 lo = reinterpret_cast<const uint2 *>(tab)[kk * n_pos + s];
+    const uint2 lo = reinterpret_cast<const uint2 *>(tab)[idx];
     w.x[0] = lo.x;
     if (NW > 1) w.x[1 % NW] = lo.y;
-    if (NW > 2) w.x[2 % NW] = reinterpret_cast<const uint32_t *>(tab + kStageSfts * n_pos * 8)[kk * n_pos + s];
+    if (NW > 2) w.x[2 % NW] = reinterpret_cast<const uint32_t *>(tab + kStageSfts * n_pos * 8)[idx];
     return w;
 }
 
@@ -183,7 +184,7 @@ __device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char 
     const double Bv[kPixTpl] = {b2.x, b2.y};
 #pragma unroll
     for (int r = 0; r < kPixTpl; ++r) {
-        int32_t s;
+        int32_t s;                                       // table index: stage row + position
         if (!CLAMP) {
             // one predicate from the FP64 compare drives both the mask update (predicated OR) and the position select
             const double g = __dsub_rn(D, Bv[r]);
@@ -197,13 +198,13 @@ __device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char 
                 "}"
                 : "+r"(brk[r]), "=r"(s)
                 : "d"(m0), "d"(mL), "n"(1u << K), "r"(k.s_zero - k.off), "r"(__double2loint(m0)));
-            s += k.off;                                  // merges with the row offset below: one uniform add
+            s += k.off + kk * n_pos;                     // position offset and stage row in one (warp-uniform) add
         } else {
             bool b;
-            s = pix_position<CLAMP>(k, D, Bv[r], b);
+            s = pix_position<CLAMP>(k, D, Bv[r], b) + kk * n_pos;
             brk[r] |= b ? (1u << K) : 0u;
         }
-        push<K, NW, HP>(cnt[r], pix_load<NW>(tab, n_pos, kk, s));
+        push<K, NW, HP>(cnt[r], pix_load<NW>(tab, n_pos, s));
     }
 }
 
