@@ -634,13 +634,15 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         const PixStage ps(pg.n_pos);
         pd.n_pg = (grid->n_pix + 31) / 32;
         pd.pix_stages = 0;
-        for (int b = 1; b < 3 && pd.pix_stages < 2; ++b) pd.pix_stages = std::min(kMaxStages, (budgets[b] - kPixHeader) / ps.stride);
+        const int hi_bytes = pix_hi_bytes(pd.NW, pd.HP);                                    // shared-memory high planes
+        for (int b = 1; b < 3 && pd.pix_stages < 2; ++b)
+            pd.pix_stages = std::min(4, (budgets[b] - kPixHeader - hi_bytes) / ps.stride);      // (2..6 stages measure alike)
         if (const char *e = getenv("BSH_STAGES")) pd.pix_stages = std::min(pd.pix_stages, std::max(2, atoi(e)));
         const bool lanes_ok = 10 * grid->n_pix >= 6 * 32 * pd.n_pg;
         pd.use_pix = !weighted && pd.pix_stages >= 2 && (lanes_ok || getenv("BSH_FORCE_PIX") != nullptr) &&
                      getenv("BSH_LEGACY") == nullptr && getenv("BSH_NO_PIX") == nullptr && !(mode & BSH_NAIVE);
         pd.pix_stages = std::max(1, std::min(pd.pix_stages, pd.n_pad / kStageSfts));
-        pd.pix_smem = kPixHeader + pd.pix_stages * ps.stride;
+        pd.pix_smem = kPixHeader + pd.pix_stages * ps.stride + hi_bytes;
         if (const char *e = getenv("BSH_SMEM_PAD")) pd.pix_smem += atoi(e);              // tuning: lowers the occupancy
     }
     pd.emit_all = pd.n_templates <= kCandCap;

@@ -309,10 +309,13 @@ struct Counter {
     uint32_t low[kLowPlanes][NW];
     uint32_t hold[kLowPlanes][NW];
     uint32_t hi[HP][NW];
+    uint32_t over[NW];                                   // carries out of the last high plane (weight 2^(5 + HP)); stays 0
+                                                         // when HP covers the SFT count, else the kernel spills it
     BSH_HD void clear()
     {
 #pragma unroll
         for (int w = 0; w < NW; ++w) {
+            over[w] = 0u;
 #pragma unroll
             for (int l = 0; l < kLowPlanes; ++l) { low[l][w] = 0u; hold[l][w] = 0u; }
 #pragma unroll
@@ -333,6 +336,8 @@ BSH_HD void push_level(Counter<NW, HP> &c, Win<NW> &x)
                 c.hi[p][w] ^= x.x[w];
                 x.x[w] = t;
             }
+#pragma unroll
+        for (int w = 0; w < NW; ++w) c.over[w] |= x.x[w];
     } else if constexpr (((K >> L) & 1) == 0) {
 #pragma unroll
         for (int w = 0; w < NW; ++w) c.hold[L][w] = x.x[w];
@@ -507,6 +512,7 @@ BSH_HD void fix_merge(Counter<NW, HP> &c, const uint32_t (&tp)[kFixPlanes][NW])
             pl = xor3(a, b, carry);
             carry = maj3(a, b, carry);
         }
+        c.over[w] |= carry;
     }
 }
 

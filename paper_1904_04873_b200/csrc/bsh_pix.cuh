@@ -29,6 +29,10 @@ constexpr int kPixTpl = 2;                           // binary templates per thr
 constexpr int kPixTile = kPixWarps * kPixTpl;        // binary templates per block
 constexpr int kPixWarpScratch = 2 * kStageSfts * kPixTpl * 8 + kPixTpl * 32;   // two B buffers + template constants
 constexpr int kPixHeader = 128 + kPixWarps * kPixWarpScratch;
+constexpr int kPixMid = 3;                           // high planes kept in registers; the other HP - 3 live in shared memory
+
+// bytes of the shared-memory high planes of one block: (HP - kPixMid) planes x 2 templates x NW words x 256 threads
+__host__ __device__ constexpr int pix_hi_bytes(int NW, int HP) { return (HP - kPixMid) * kPixTpl * NW * 32 * kPixWarps * 4; }
 
 // D table for the pixel-lane kernel: dpix[pg][i / 2][lane][i & 1] = v_i . n_pix / c (canonical order, R-5) for pixel
 // pg * 32 + lane; padding SFTs get 0, padding lanes repeat the last real pixel (never written out).  One LDS.128 per
@@ -175,7 +179,7 @@ __device__ __forceinline__ Win<NW> pix_load(const unsigned char *tab, int n_pos,
 // One SFT (slot K of the unrolled block of 32) for both templates of the thread.
 template <int K, int NW, int HP, bool CLAMP>
 __device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char *tab, int n_pos, const double2 *bpair,
-                                         const double2 *dpair, Counter<NW, HP> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl])
+                                         const double2 *dpair, Counter<NW, kPixMid> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl])
 {
     constexpr int kk = K % kStageSfts;
     const double2 d2 = dpair[(kk >> 1) * 32];
@@ -204,13 +208,13 @@ __device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char 
             s = pix_position<CLAMP>(k, D, Bv[r], b) + kk * n_pos;
             brk[r] |= b ? (1u << K) : 0u;
         }
-        push<K, NW, HP>(cnt[r], pix_load<NW>(tab, n_pos, s));
+        push<K, NW, kPixMid>(cnt[r], pix_load<NW>(tab, n_pos, s));
     }
 }
 
 template <int K0, int NW, int HP, bool CLAMP, int... Ks>
 __device__ __forceinline__ void pix_half(const PixConst &k, const unsigned char *tab, int n_pos, const double2 *bpair,
-                                         const double2 *dpair, Counter<NW, HP> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl],
+                                         const double2 *dpair, Counter<NW, kPixMid> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl],
                                          std::integer_sequence<int, Ks...>)
 {
     (pix_step<K0 + Ks, NW, HP, CLAMP>(k, tab, n_pos, bpair, dpair, cnt, brk), ...);
@@ -276,7 +280,31 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
     kc.s_max = p.s_max;
     kc.s_zero = p.s_zero;
 
-    Counter<NW, HP> cnt[kPixTpl];
+    // Counters: 5 low planes (carry-save tree over a block of 32 SFTs) + kPixMid planes in registers; the HP - kPixMid
+    // planes above live in shared memory, [plane][template][word][thread].  A register counter wraps at most once in 8
+    // blocks (one carry of weight 32 per block), so its carries-out are OR-ed into `over` and rippled into the shared
+    // planes every 8th block (and around every fix-up merge): 66 -> 48 counter registers, no spills at any SFT count.
+    constexpr int HS = HP - kPixMid;
+    uint32_t *hs = reinterpret_cast<uint32_t *>(smem + kPixHeader + p.n_stages * L.stride) + threadIdx.x;
+    constexpr int kHsStride = 32 * kPixWarps;
+#pragma unroll
+    for (int q = 0; q < HS * kPixTpl * NW; ++q) hs[q * kHsStride] = 0u;
+    auto spill_over = [&](Counter<NW, kPixMid> &c, int r) {
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+            uint32_t carry = c.over[w];
+#pragma unroll
+            for (int q = 0; q < HS; ++q) {
+                uint32_t *pl = hs + ((q * kPixTpl + r) * NW + w) * kHsStride;
+                const uint32_t t = *pl;
+                *pl = t ^ carry;
+                carry = t & carry;
+            }
+            c.over[w] = 0u;
+        }
+    };
+
+    Counter<NW, kPixMid> cnt[kPixTpl];
     uint16_t list[kPixTpl][kListCap];
     int npend[kPixTpl];
 #pragma unroll
@@ -343,9 +371,15 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
                     const double D = p.dpix[((((int64_t)pg * (p.n_pad >> 1)) + (i >> 1)) * 32 + lane) * 2 + (i & 1)];
                     fix_accumulate<NW>(tp, exact_window_pos<NW, CLAMP>(tc, p.ptab + (int64_t)i * p.n_pos, D, B));
                 }
-                fix_merge<NW, HP>(cnt[r], tp);
+                spill_over(cnt[r], r);                   // `over` must be empty: the merge may carry out of plane 7
+                fix_merge<NW, kPixMid>(cnt[r], tp);
+                spill_over(cnt[r], r);
                 npend[r] = 0;
             }
+        }
+        if ((blk & 7) == 7 || blk + 1 == n_blocks) {
+#pragma unroll
+            for (int r = 0; r < kPixTpl; ++r) spill_over(cnt[r], r);
         }
     }
 
@@ -355,15 +389,25 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
 #pragma unroll
     for (int r = 0; r < kPixTpl; ++r) {
         if (!act[r] || pix >= p.n_pix) continue;
+        Counter<NW, HP> full_cnt;                        // all 5 + HP planes of this template, for the comparisons below
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+#pragma unroll
+            for (int l = 0; l < kLowPlanes; ++l) full_cnt.low[l][w] = cnt[r].low[l][w];
+#pragma unroll
+            for (int q = 0; q < kPixMid; ++q) full_cnt.hi[q][w] = cnt[r].hi[q][w];
+#pragma unroll
+            for (int q = 0; q < HS; ++q) full_cnt.hi[kPixMid + q][w] = hs[((q * kPixTpl + r) * NW + w) * kHsStride];
+        }
         const uint64_t base =
             ((((uint64_t)pix * p.n_ap + ia[r]) * p.n_P + ip) * p.n_tasc + it[r]) * (uint64_t)p.n_f0 + p.j0;
-        const Win<NW> ge = count_ge(cnt[r], tau);
+        const Win<NW> ge = count_ge(full_cnt, tau);
         int32_t *out = p.counts_full ? reinterpret_cast<int32_t *>(p.counts_full) + base : nullptr;
 #pragma unroll
         for (int w = 0; w < NW; ++w) {
             if (out) {
                 for (int bb = 0; bb < 32; ++bb)
-                    if (32 * w + bb < p.n_fj) out[32 * w + bb] = count_at(cnt[r], w, bb);
+                    if (32 * w + bb < p.n_fj) out[32 * w + bb] = count_at(full_cnt, w, bb);
             }
             uint32_t m = ge.x[w] & valid_mask(p.n_fj, w);
             while (m) {
@@ -373,7 +417,7 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
                 if (pos < p.cand_cap) {
                     RawCand rc;
                     rc.index = base + 32 * w + bb;
-                    rc.key = (uint32_t)count_at(cnt[r], w, bb);
+                    rc.key = (uint32_t)count_at(full_cnt, w, bb);
                     rc.pad = 0u;
                     p.cand[pos] = rc;
                 }
