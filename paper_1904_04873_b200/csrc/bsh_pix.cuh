@@ -29,7 +29,8 @@ constexpr int kPixTpl = 2;                           // binary templates per thr
 constexpr int kPixTile = kPixWarps * kPixTpl;        // binary templates per block
 constexpr int kPixWarpScratch = 2 * kStageSfts * kPixTpl * 8 + kPixTpl * 32;   // two B buffers + template constants
 constexpr int kPixHeader = 128 + kPixWarps * kPixWarpScratch;
-constexpr int kPixMid = 3;                           // high planes kept in registers; the other HP - 3 live in shared memory
+constexpr int kPixMid = 2;                           // high planes kept in registers (the other HP - 2 live in shared
+                                                     // memory); 3 and 4 measured 2 % and 5 % slower on config 2
 
 // bytes of the shared-memory high planes of one block: (HP - kPixMid) planes x 2 templates x NW words x 256 threads
 __host__ __device__ constexpr int pix_hi_bytes(int NW, int HP) { return (HP - kPixMid) * kPixTpl * NW * 32 * kPixWarps * 4; }
@@ -281,9 +282,10 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
     kc.s_zero = p.s_zero;
 
     // Counters: 5 low planes (carry-save tree over a block of 32 SFTs) + kPixMid planes in registers; the HP - kPixMid
-    // planes above live in shared memory, [plane][template][word][thread].  A register counter wraps at most once in 8
-    // blocks (one carry of weight 32 per block), so its carries-out are OR-ed into `over` and rippled into the shared
-    // planes every 8th block (and around every fix-up merge): 66 -> 48 counter registers, no spills at any SFT count.
+    // planes above live in shared memory, [plane][template][word][thread].  A register counter wraps at most once in
+    // 2^kPixMid blocks (one carry of weight 32 per block), so its carries-out are OR-ed into `over` and rippled into the
+    // shared planes every 2^kPixMid-th block (and around every fix-up merge): 66 -> 42 counter registers, no spills at
+    // any SFT count.
     constexpr int HS = HP - kPixMid;
     uint32_t *hs = reinterpret_cast<uint32_t *>(smem + kPixHeader + p.n_stages * L.stride) + threadIdx.x;
     constexpr int kHsStride = 32 * kPixWarps;
@@ -377,7 +379,7 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
                 npend[r] = 0;
             }
         }
-        if ((blk & 7) == 7 || blk + 1 == n_blocks) {
+        if ((blk & ((1 << kPixMid) - 1)) == (1 << kPixMid) - 1 || blk + 1 == n_blocks) {
 #pragma unroll
             for (int r = 0; r < kPixTpl; ++r) spill_over(cnt[r], r);
         }

@@ -202,7 +202,7 @@ def test_multiple_breaks_per_band_fallback(bsh, torch, ctx):
 # ------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n_sft,n_f0,margin,f0,side", [(1, 1, 3, 50.0, 1), (33, 7, 12, 80.0, 3), (64, 90, 30, 120.0, 6),
                                                         (130, 97, 45, 150.0, 6), (70, 200, 60, 200.0, 3),
-                                                        (2100, 64, 50, 180.0, 6)])
+                                                        (2100, 64, 50, 180.0, 6), (8200, 33, 45, 150.0, 3)])
 def test_pixel_lane_kernel_ragged(bsh, torch, ctx, monkeypatch, n_sft, n_f0, margin, f0, side):
     wl = synth.noise_workload(seed=1000 + n_sft + n_f0, n_sft=n_sft, n_f0=n_f0, margin=margin, f_band_start=f0,
                               n_pix_side=side, ap=(10.0, 40.0), P_days=(15.0, 31.0), n_t=3, topk=7)
