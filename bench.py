@@ -55,7 +55,7 @@ OPS_PER_TRIPLE_WEIGHTED_FIXED = 19.0
 OPS_PER_ACC_WEIGHTED = 2.0
 GATHER_LANES_PER_SM_CLK = 32      # north_star bound (b) read literally: one 4-byte lane-gather per accumulation
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the kernel (ncu --set full, profiles/r01d_stage1_pix_full.md)
-NCU_DRAM_BYTES_PER_LAUNCH = 12728832 + 670464
+NCU_DRAM_BYTES_PER_LAUNCH = 13085184 + 598784
 
 
 def measured_peaks():
