@@ -52,6 +52,7 @@ struct Pending {                      // state between bsh_stage1_launch and bsh
     uint64_t n_templates = 0;
     bool emit_all = false, clamp = false;
     int tile_bins = 96;               // f0 bins per accumulation pass (<= 32 NW)
+    unsigned int cand_cap = kCandCap; // candidate buffer entries of this call (grows with topk: fraction-N_C toplists, L225)
     int R = 2, NW = 3, HP = 6, n_entries = 0, off_table = 0, s_max = 0, s_zero = 0, list_cap = 0, tpb = 256, n_groups = 0, n_aq_tiles = 0;
     double frac = 0, shift_sigma = 0;
     int passes = 0;
@@ -345,7 +346,7 @@ int run_pass(bsh_ctx *ctx)
         if (blocks > 0x7FFFFFFFull) return fail(ctx, BSH_EINVAL, "naive kernel: too many templates");
         stage1_naive_kernel<<<(unsigned)blocks, 256, 0, ctx->stream>>>(
             t, pd.d_peak, pd.words_per_row, pd.d_w, weighted ? 1 : 0, pd.n_templates, (const Threshold *)ctx->thr.p,
-            (RawCand *)ctx->cand.p, (unsigned int *)ctx->cand_count.p, kCandCap, pd.d_counts_full);
+            (RawCand *)ctx->cand.p, (unsigned int *)ctx->cand_count.p, pd.cand_cap, pd.d_counts_full);
         count_launch(ctx);
         CK(cudaGetLastError());
         ctx->st.grid_blocks = (int)blocks;
@@ -371,7 +372,7 @@ int run_pass(bsh_ctx *ctx)
             p.thr = (const Threshold *)ctx->thr.p;
             p.cand = (RawCand *)ctx->cand.p;
             p.cand_count = (unsigned int *)ctx->cand_count.p;
-            p.cand_cap = kCandCap;
+            p.cand_cap = pd.cand_cap;
             p.counts_full = pd.d_counts_full;
             const int64_t grid = (int64_t)pd.n_pg * pd.n_P * p.n_aq_tiles;
             if (grid > 0x7FFFFFFFll) return fail(ctx, BSH_EINVAL, "grid too large");
@@ -400,7 +401,7 @@ int run_pass(bsh_ctx *ctx)
             p.thr = (const Threshold *)ctx->thr.p;
             p.cand = (RawCand *)ctx->cand.p;
             p.cand_count = (unsigned int *)ctx->cand_count.p;
-            p.cand_cap = kCandCap;
+            p.cand_cap = pd.cand_cap;
             p.counts_full = pd.d_counts_full;
             const int64_t grid = (int64_t)pd.n_oct * pd.n_P * p.n_aq_tiles;
             if (grid > 0x7FFFFFFFll) return fail(ctx, BSH_EINVAL, "grid too large");
@@ -430,7 +431,7 @@ int run_pass(bsh_ctx *ctx)
             p.thr = (const Threshold *)ctx->thr.p;
             p.cand = (RawCand *)ctx->cand.p;
             p.cand_count = (unsigned int *)ctx->cand_count.p;
-            p.cand_cap = kCandCap;
+            p.cand_cap = pd.cand_cap;
             p.counts_full = pd.d_counts_full;
             const int64_t grid = (int64_t)pd.n_groups * pd.n_P * pd.n_aq_tiles;
             if (grid > 0x7FFFFFFFll) return fail(ctx, BSH_EINVAL, "grid too large");
@@ -645,9 +646,17 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         pd.pix_smem = kPixHeader + pd.pix_stages * ps.stride + hi_bytes;
         if (const char *e = getenv("BSH_SMEM_PAD")) pd.pix_smem += atoi(e);              // tuning: lowers the occupancy
     }
-    pd.emit_all = pd.n_templates <= kCandCap;
+    // Toplists as large as a fraction N_C of the bank (L225: 5-10 % of all templates go to stage 2) need a larger
+    // candidate buffer and a tighter first guess of the threshold (1.3 k instead of 8 k expected survivors).
+    pd.cand_cap = kCandCap;
+    if ((uint64_t)topk > kCandCap / 8) {
+        const uint64_t need = std::min<uint64_t>(pd.n_templates, 4ull * (uint64_t)topk);
+        while (pd.cand_cap < need && pd.cand_cap < (1u << 27)) pd.cand_cap <<= 1;
+    }
+    pd.emit_all = pd.n_templates <= pd.cand_cap;
     pd.frac = (double)std::max<int64_t>(8ll * topk, 4096) / (double)pd.n_templates;
-    if (pd.frac >= 0.25) pd.frac = 0.25;
+    if ((uint64_t)topk > kCandCap / 8) pd.frac = (1.3 * (double)topk + 4096.0) / (double)pd.n_templates;
+    if (pd.frac >= 0.25) pd.frac = (uint64_t)topk > kCandCap / 8 ? std::min(pd.frac, 0.45) : 0.25;
     pd.shift_sigma = 0.0;
     pd.passes = 0;
 
@@ -656,7 +665,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     TRY(ensure(ctx, ctx->w_pad, (size_t)pd.n_pad * 4));
     TRY(ensure(ctx, ctx->stats, 16));
     TRY(ensure(ctx, ctx->thr, sizeof(Threshold)));
-    TRY(ensure(ctx, ctx->cand, (size_t)kCandCap * sizeof(RawCand)));
+    TRY(ensure(ctx, ctx->cand, (size_t)pd.cand_cap * sizeof(RawCand)));
     TRY(ensure(ctx, ctx->cand_count, 16));
 
     CK(cudaEventRecord(ctx->ev[0], ctx->stream));
@@ -731,7 +740,7 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
     for (;;) {
         CK(cudaStreamSynchronize(ctx->stream));
         n_cand = ctx->pinned_count[0];
-        const bool too_few = n_cand < want, too_many = n_cand > kCandCap;
+        const bool too_few = n_cand < want, too_many = n_cand > pd.cand_cap;
         if (!too_few && !too_many) break;
         if (pd.passes >= kMaxPasses) return fail(ctx, BSH_ECUDA, "candidate selection did not converge (%u candidates)", n_cand);
         float ms = 0.f;
@@ -757,7 +766,7 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
     RawCand *sorted = (RawCand *)ctx->cand.p;
     if (n_cand > (unsigned)kSortTile && (uint64_t)n_cand > want && getenv("BSH_FULL_SORT") == nullptr) {
         // only the candidates at or above the k-th largest key take part in the sort (ties at the cut included)
-        TRY(ensure(ctx, ctx->keys, (size_t)kCandCap * sizeof(RawCand)));
+        TRY(ensure(ctx, ctx->keys, (size_t)pd.cand_cap * sizeof(RawCand)));
         select_cut_kernel<<<1, 1024, 0, ctx->stream>>>((const RawCand *)ctx->cand.p, n_cand, (unsigned int)want,
                                                        (RawCand *)ctx->keys.p, (unsigned int *)ctx->cand_count.p + 1);
         count_launch(ctx);

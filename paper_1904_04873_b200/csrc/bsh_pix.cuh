@@ -6,12 +6,14 @@
 // pair of binary templates and 32 neighbouring sky pixels:
 //   * the pixels of a patch are less than one frequency bin apart per pixel step (Eq. 34), so the 32 positions
 //     of a warp fall into a handful of consecutive table entries: same entry -> broadcast, neighbours -> different
-//     banks.  The window read costs 2 wavefronts instead of 5;
+//     banks (ncu: 136 M -> 20 M bank conflicts); the window is read as LDS.64 + LDS.32 from a split table;
 //   * the binary term B = A (C CA + S SA) of Eq. (15) (L102) is the same for all lanes.  Each lane computes ONE of the
 //     warp's 2 x 16 values per stage and the warp shares them through shared memory, so the hot loop spends no FP64
-//     work on it (9 -> 7 FP64 operations per (pixel, template, SFT) triple);
+//     work on it: g = D - B, y at both band ends, two rounding adds, one compare = 6 FP64 operations per (pixel,
+//     template, SFT) triple;
 //   * breaks of the rounded shift inside the f0 tile (R-7) are flagged by comparing the two magic-add results as
-//     doubles (FP64 pipe, not the integer pipe) and recorded in a 32-bit mask per block of 32 SFTs.
+//     doubles (FP64 pipe, not the integer pipe) and recorded in a 32-bit mask per block of 32 SFTs;
+//   * the bit-sliced counters are two-level: 5 + 2 planes in registers, the planes above in shared memory.
 // Thread = 1 pixel x 2 templates x up to 32 NW f0 bins; block = 8 warps = 16 templates of one period, 32 pixels.
 //
 //   PAPER.md L102 Eq. (15) track, L223 number count, L241-L247 "loop over the binary templates"; R-5, R-7.

@@ -373,3 +373,18 @@ def tie_workload() -> Workload:
                     n_bins=n_f0 + 2 * margin, k_band0=k_band0, n_f0=n_f0, rho=np.ascontiguousarray(rho),
                     w=np.ones(n, np.float32), alpha=np.zeros(1), delta=np.zeros(1), ap=np.zeros(1),
                     P=np.array([15.0 * DAY]), tasc_frac=np.zeros(1), topk=4)
+
+
+def overlapped_stage2_set(wl: Workload, seed: int = 0, lat_deg: float = 30.6, theta0: float = 0.0) -> Workload:
+    """Stage-2 SFT set of PAPER.md L233: the stage-1 SFTs plus a second set whose start times are shifted by T_sft / 2
+    (N-bar ~ 2 N in Table I).  Same template grid, same time origin and the SAME t_search_mid as `wl` (the templates
+    -- their t_asc -- must not move); fresh Exp(1) powers and log-normal weights for the 2 N rows.  Single-detector
+    velocity model (the test workloads it is used with are single-detector)."""
+    t1 = np.asarray(wl.t_mid, np.float64)
+    t2 = np.sort(np.concatenate([t1, t1 + 0.5 * wl.t_sft]))
+    rng = _rng(seed, 77)
+    n2 = t2.shape[0]
+    # t_mid is relative to the first SFT start; the velocity model wants absolute mid-times with the same origin
+    v2 = detector_velocity_over_c(t2, lat_deg, theta0)
+    return dataclasses.replace(wl, name=wl.name + "-stage2", t_mid=np.ascontiguousarray(t2), v_over_c=v2,
+                               rho=exp_powers(rng, n2, wl.n_bins), w=lognormal_weights(rng, n2))

@@ -443,3 +443,56 @@ def test_ties_round_to_even_on_the_gpu(bsh, torch, ctx, monkeypatch):
         assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=0), env
     r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED | bsh.BSH_NAIVE)
     assert np.array_equal(r["counts"], want_n)
+
+
+def test_stage2_on_half_overlapped_sft_set(bsh, torch, ctx):
+    """PAPER.md L233 / SURVEY NEXT-1: stage 2 re-scores the stage-1 toplist on a DIFFERENT SFT set (the stage-1 SFTs plus
+    a set shifted by T/2: 2 N rows, other velocities, powers and weights), same templates."""
+    wl = synth.noise_workload(seed=501, n_sft=300, n_f0=90, margin=45, f_band_start=150.0, n_pix_side=6,
+                              ap=(10.0, 25.0, 40.0), P_days=(15.0, 31.0), n_t=4, topk=200)
+    wl2 = synth.overlapped_stage2_set(wl, seed=502)
+    assert wl2.n_sft == 2 * wl.n_sft and wl2.t_search_mid == wl.t_search_mid
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=200, full=False)
+    d_rho2, d_w2 = dev(torch, wl2.rho), dev(torch, wl2.w)
+    ctx.stage2_power(d_rho2, wl2, r["d_top"], 200, d_w=d_w2, sort_by_power=True)
+    torch.cuda.synchronize()
+    recs = ctx.records(r["d_top"], 200)
+    want = oracle.stage2(wl2, recs["index"], wl2.rho, wl2.w)
+    assert np.allclose(recs["power"], want, rtol=RTOL, atol=0)
+    assert np.all(np.diff(recs["power"]) <= 0), "sorted by power, best first"
+    assert set(recs["index"].tolist()) == set(r["top"]["index"].tolist()), "same candidates, new order"
+
+
+def test_fraction_nc_toplist_and_stage2(bsh, torch, ctx):
+    """PAPER.md L225-L233 / SURVEY NEXT-1: the toplist is a FRACTION N_C = 5 % of all templates of the patch (here 5.6e5 of
+    1.1e7, beyond the default candidate buffer), and stage 2 re-scores all of them on the half-overlapped SFT set.
+    The full count dump is checked against the oracle on sampled templates; the toplist must be exactly the top-k of the
+    dump by (count desc, index asc); powers are checked against the oracle on sampled candidates."""
+    wl = synth.noise_workload(seed=601, n_sft=500, n_f0=90, margin=45, f_band_start=150.0, n_pix_side=8,
+                              ap=tuple(np.linspace(10.0, 40.0, 8)), P_days=tuple(np.linspace(15.0, 45.0, 12)), n_t=20,
+                              topk=10)
+    assert wl.n_templates == 64 * 8 * 12 * 20 * 90
+    k = int(0.05 * wl.n_templates)
+    assert k > (1 << 20) // 2
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=k, full=True)
+    assert r["n_top"] == k
+    dump = r["counts"]
+    rng = np.random.default_rng(5)
+    pk = oracle.peakgram(wl.rho)
+    sample = np.unique(rng.integers(0, wl.n_templates, 3000)).astype(np.uint64)
+    want_n, _, _ = oracle.score(wl, sample, peak=pk, w=wl.w)
+    assert np.array_equal(dump[sample.astype(np.int64)], want_n)
+    want_top = np.lexsort((np.arange(dump.size), -dump.astype(np.int64)))[:k]
+    assert np.array_equal(r["top"]["index"].astype(np.int64), want_top)
+    assert np.array_equal(r["top"]["count"], dump[want_top])
+    # stage 2 on all N_C candidates, on the half-overlapped set
+    wl2 = synth.overlapped_stage2_set(wl, seed=602)
+    d_rho2, d_w2 = dev(torch, wl2.rho), dev(torch, wl2.w)
+    ctx.stage2_power(d_rho2, wl2, r["d_top"], k, d_w=d_w2, sort_by_power=True)
+    torch.cuda.synchronize()
+    recs = ctx.records(r["d_top"], k)
+    assert np.all(np.diff(recs["power"]) <= 0)
+    assert np.array_equal(np.sort(recs["index"]), np.sort(r["top"]["index"]))
+    pick = np.unique(np.concatenate([np.arange(200), rng.integers(0, k, 2000)]))
+    want_p = oracle.stage2(wl2, recs["index"][pick], wl2.rho, wl2.w)
+    assert np.allclose(recs["power"][pick], want_p, rtol=RTOL, atol=0)
