@@ -481,7 +481,7 @@ BSH_HD Win<NW> exact_window_pos(const TrackConst &tc, const uint4 *row_positions
 
 // The deferred windows of one flush are first summed in a small bit-sliced accumulator (kFixPlanes planes, ripple
 // carry: 2 kFixPlanes LOP per word and window instead of 2 (5 + HP)), which is then added to the counter once.
-constexpr int kFixPlanes = 7;                            // up to 127 windows per flush (kListCap = 64)
+constexpr int kFixPlanes = 7;                            // up to 127 windows per flush (kListCap = 120)
 
 template <int NW>
 BSH_HD void fix_accumulate(uint32_t (&tp)[kFixPlanes][NW], const Win<NW> &x)

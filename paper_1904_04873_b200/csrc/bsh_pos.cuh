@@ -24,7 +24,10 @@ namespace bsh {
 constexpr int kStageSfts = 16;        // SFTs per shared-memory stage (half an unrolled block of 32)
 constexpr int kMaxStages = 6;
 constexpr int kPosHeader = 128;       // full[kMaxStages] mbarriers + done[kMaxStages] counters
-constexpr int kListCap = 64;          // deferred breaks per (thread, pixel); flushed when more than 32 are pending
+constexpr int kListCap = 120;         // deferred breaks per (thread, template or pixel); flushed when more than 88 are
+                                      // pending (< 2^kFixPlanes windows per flush).  64 measured 25-30 % slower at 8000 SFTs:
+                                      // a flush is a long latency-bound loop during which the block's other warps run
+                                      // out of staged SFTs, so fewer and fuller flushes win
 constexpr int kWarpsUnweighted = 8;   // warps per block = pixel groups per block
 #ifndef BSH_W_UNROLL
 #define BSH_W_UNROLL 16
