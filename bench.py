@@ -1,15 +1,23 @@
 #!/usr/bin/env python
-"""bench.py -- template x SFT Hough accumulations per second on the BASELINE.json config-2 sky patch.
+"""bench.py -- template x SFT Hough accumulations per second of the BinarySkyHough hot path on one B200.
 
-One STEP = one pass of the whole hot path over one sky patch (BASELINE.json configs[1]: 2000 SFTs, 8x8 pixels,
-20 x 30 x 40 binary templates, 90 f0 bins = 1.3824e8 templates, 2.7648e11 accumulations):
-    bsh_build_peakgram -> bsh_stage1_hough (unweighted number count + top-1000) -> bsh_stage2_power (re-score + sort)
-with the normalised powers already resident in HBM.  `value` = accumulations of all ranks / device time (max over ranks).
+One STEP = one pass of the whole hot path over one sky patch, normalised powers already resident in HBM:
+    bsh_build_peakgram -> bsh_stage1_hough (number count of every template + top-1000) -> bsh_stage2_power (re-score, sort)
+
+    --config 3 (default)  BASELINE.json configs[2], the full-size search patch: 8000 SFTs (two detectors x 4000, 30 % gaps),
+                          8x8 pixels, 40 x 60 x 120 binary templates, 90 f0 bins = 1.659e9 templates, 1.327e13 accumulations;
+                          WEIGHTED FP32 number count (Eq. 22) -- the headline `value`.
+    --config 2            configs[1]: 2000 SFTs, 1.3824e8 templates; unweighted count is the headline of that line.
+    --config 5            configs[4]: sweep over sky patches of the 256-patch hemisphere tiling on two CUDA streams.
+
+The default line also carries, as named sub-objects, the unweighted count on the same patch, config 2 (both counts), a
+config-5 sweep over 32 patches, the fraction-N_C toplist and the front end (NEXT-2) timings.
 `e2e` = the same patch through bsh_search_patch_host() with HOST buffers (H2D of rho and w, D2H of the toplist inside the
-timed region).  `roofline` describes the dominant kernel (stage-1 accumulation); `cpu_baseline` is the plain oracle
-(oracle/, Eq. 15 with one cos per accumulation) timed on this box's host cores on a bounded sub-grid.
+timed region).  `roofline` describes the dominant kernel (the stage-1 accumulation of the headline mode) against on-chip
+peaks MEASURED in the same run (bsh_measure_peaks).  `cpu_baseline` is the plain oracle (oracle/, Eq. 15 with one cos per
+accumulation) timed on this box's host cores on a bounded sub-grid, all cores and single-threaded.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python bench.py [--config 3|2|5] [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
 For N > 1 launch under torchrun (one rank per GPU); ranks process different seeded patches, no data-path collective
 (weak scaling, DESIGN.md section "Multi-GPU").
 """
@@ -32,33 +40,27 @@ import synth  # noqa: E402
 METRIC = "template*SFT Hough accumulations/sec"
 UNIT = "accumulations/s"
 
-# --- roofline model of the stage-1 accumulation kernel -----------------------------------------
-# Unit of work: one (pixel, binary template, SFT) TRIPLE = n_f0 (90) accumulations.  The kernel is bound on chip by plain
-# instruction throughput: every pipe it uses (integer ALU, FP64, LSU/shared memory) is 40-60 % busy and the warp
-# schedulers issue 63 % of their slots (ncu, profiles/r01d_stage1_pix_full.md); HBM is idle.  Roofline = warp-issue peak.
-N_SM = 148
-LANES_PER_SM_CLK = 128            # 4 SMSPs x 32 lanes: one warp instruction per scheduler per clock
-# algorithmic lane-instructions per triple -- what this formulation must execute whatever the schedule:
+# --- roofline models of the stage-1 accumulation kernels ----------------------------------------
+# Weighted count ("the weighted sum of 1s and 0s"): the method's work is ONE FP32 add per accumulation
+# (template x SFT); everything else (track, predicates, staging) is overhead of the formulation.  Bound: the FP32-add
+# pipe, peak = measured predicated-FADD lanes/clk/SM x SMs x clock.
+# Unweighted count: unit of work = one (pixel, binary template, SFT) TRIPLE = n_f0 (90) accumulations sharing one
+# track evaluation and one 96-bit window; bound by plain instruction issue.  Algorithmic lane-instructions per triple:
 #   FP64  g = D - B (1), y at both band ends (2), round by magic add (2), equal-shift test (1)                      6
 #   count 3 window words x full adder (2 LOP3) + ripple into the 6 high planes once per 32 SFTs (36 / 32)           7.125
 #   INT   position select on a break (1), break mask (1), shared-memory address (1)                                 3
 #   LSU   window read (LDS.64 + LDS.32) 2, binary terms of 2 templates per load 0.5, Doppler terms of 2 SFTs
 #         per load shared by 2 templates 0.25                                                                       2.75
 ALGO_OPS_PER_TRIPLE = 6.0 + 7.125 + 3.0 + 2.75
-# secondary views: the shared-memory data pipe (one 128-byte wavefront per clock per SM) and the integer-ALU pipe alone
-SMEM_BYTES_PER_CLK_SM = 128
 SMEM_BYTES_PER_TRIPLE = 12.0 + 4.0 + 4.0      # 96-bit window + D (8 B per 2 templates) + B (one wavefront per 32 triples)
-ALU_LANES_PER_SM_CLK = 64                      # 16 lanes/clk/SMSP (B300_MICROARCH.md: alu-pipe rt_SMSP = 2)
-ALU_OPS_PER_TRIPLE = 6.0 + 1.125 + 3.0
-# weighted kernel: one predicated FP32 add + one predicate-generating op per accumulation, plus the track per triple
-OPS_PER_TRIPLE_WEIGHTED_FIXED = 19.0
-OPS_PER_ACC_WEIGHTED = 2.0
-GATHER_LANES_PER_SM_CLK = 32      # north_star bound (b) read literally: one 4-byte lane-gather per accumulation
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the kernel (ncu --set full, profiles/r01d_stage1_pix_full.md)
-NCU_DRAM_BYTES_PER_LAUNCH = 13085184 + 598784
+ALU_OPS_PER_TRIPLE = 6.0 + 1.125 + 3.0         # the integer-ALU pipe's share of the above
+GATHER_LANES_PER_SM_CLK = 32                   # north_star bound (b) read literally: one 4-byte lane-gather per accumulation
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
+NCU_DRAM_BYTES = {"weighted": None, "unweighted": None}
+NCU_DRAM_SOURCE = "profiles/ (no capture of this kernel yet)"
 
 
-def measured_peaks():
+def measured_peaks_file():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
             return json.load(fh)
@@ -118,50 +120,73 @@ def physical_gpu_index(local: int) -> int:
     return local
 
 
+def workload_for(config: int, rank: int = 0):
+    if config == 2:
+        return synth.config2(seed=2 + rank), "config2 (BASELINE.json configs[1])"
+    if config == 3:
+        return synth.config3(seed=3 + 100 * rank), "config3 (BASELINE.json configs[2])"
+    c5 = synth.config5(seed=5 + 100 * rank)
+    return c5, "config5 (BASELINE.json configs[4])"
+
+
 # ---------------------------------------------------------------------------------------------------------------------
 # reference arm / cpu baseline: the plain oracle on a bounded sample of the same workload
 # ---------------------------------------------------------------------------------------------------------------------
-def oracle_sample(wl, target_seconds: float):
-    """Times oracle.stage1 (DIRECT: Eq. 15 with one libm cos per accumulation, OpenMP over templates) on a sub-grid of the
-    workload: all 90 f0 bins and all SFTs, a few pixels x binary templates, sized to ~target_seconds."""
+def oracle_subgrid(wl, seconds: float, n_threads: int = 0):
+    """A sub-grid of the workload (all f0 bins and all SFTs, a few pixels x binary templates) that the oracle's DIRECT
+    mode (Eq. 15 with one libm cos per accumulation) finishes in ~`seconds` on n_threads (0 = all cores)."""
     import oracle
     pk = oracle.peakgram(wl.rho)
     probe = wl.subgrid(ia=[0], ip=[0], it=[0, 1], pix=[0, 1])
     t0 = time.perf_counter()
-    oracle.stage1(probe, pk, wl.w, mode=oracle.DIRECT)
+    oracle.stage1(probe, pk, wl.w, mode=oracle.DIRECT, n_threads=n_threads)
     rate = probe.n_accumulations / max(time.perf_counter() - t0, 1e-6)
-    n_b = int(max(2, min(wl.n_binary * wl.n_pix, rate * target_seconds / (wl.n_f0 * wl.n_sft))))
+    n_b = int(max(2, min(wl.n_binary * wl.n_pix, rate * seconds / (wl.n_f0 * wl.n_sft))))
     n_it = min(len(wl.tasc_frac), max(1, n_b // 8))
     n_pix = min(wl.n_pix, max(1, n_b // n_it))
-    sub = wl.subgrid(ia=[0], ip=[0], it=list(range(n_it)), pix=list(range(n_pix)))
-    return sub, pk
+    return wl.subgrid(ia=[0], ip=[0], it=list(range(n_it)), pix=list(range(n_pix))), pk
 
 
-def run_oracle_steps(wl, steps: int, warmup: int, seconds_per_step: float):
+def run_oracle_steps(wl, label, steps: int, warmup: int, seconds_per_step: float, n_threads: int = 0):
+    """`steps` passes of the oracle's whole path (stage 1 of every template of the sub-grid, toplist by full sort, stage 2)."""
     import oracle
-    sub, pk = oracle_sample(wl, seconds_per_step)
+    sub, pk = oracle_subgrid(wl, seconds_per_step, n_threads)
     for _ in range(min(warmup, 1)):
-        oracle.stage1(sub, pk, wl.w, mode=oracle.DIRECT)
+        oracle.stage1(sub, pk, wl.w, mode=oracle.DIRECT, n_threads=n_threads)
     t0 = time.perf_counter()
     for _ in range(steps):
-        cnt, _ = oracle.stage1(sub, pk, wl.w, mode=oracle.DIRECT)
-        top = oracle.toplist(cnt.astype(np.float64), min(wl.topk, cnt.size))
-        oracle.stage2(sub, top, wl.rho, wl.w, mode=oracle.DIRECT)
+        cnt, wc = oracle.stage1(sub, pk, wl.w, mode=oracle.DIRECT, n_threads=n_threads)
+        top = oracle.toplist(wc, min(wl.topk, cnt.size))
+        oracle.stage2(sub, top, wl.rho, wl.w, mode=oracle.DIRECT, n_threads=n_threads)
     dt = time.perf_counter() - t0
-    sample = (f"oracle DIRECT mode on a sub-grid of config 2: {sub.n_pix} pixels x {sub.n_binary} binary templates x "
+    cores = n_threads if n_threads > 0 else oracle.max_threads()
+    sample = (f"oracle DIRECT mode on a sub-grid of {label}: {sub.n_pix} pixels x {sub.n_binary} binary templates x "
               f"{sub.n_f0} f0 x {sub.n_sft} SFTs = {sub.n_accumulations:.3e} accumulations per step")
-    return steps * sub.n_accumulations / dt, dt / steps, oracle.max_threads(), sample
+    return steps * sub.n_accumulations / dt, dt / steps, cores, sample
+
+
+def cpu_baseline(wl, label):
+    """All host cores (~12 s) and one thread (~6 s), same oracle, same inputs; extrapolation flagged as such."""
+    value, _, cores, sample = run_oracle_steps(wl, label, 1, 0, seconds_per_step=12.0)
+    v1, _, _, sample1 = run_oracle_steps(wl, label, 1, 0, seconds_per_step=6.0, n_threads=1)
+    return {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+            "single_thread": {"value": v1, "unit": UNIT, "cores": 1, "sample": sample1},
+            "extrapolated_full_config_seconds": {"all_cores": wl.n_accumulations / value,
+                                                 "single_thread": wl.n_accumulations / v1,
+                                                 "note": "EXTRAPOLATED linearly from the sub-grid rate to the full config"}}
 
 
 def main_reference(args, rank, world):
     if rank != 0:
         return
-    wl = synth.config2()
-    value, s_per_step, cores, sample = run_oracle_steps(wl, args.steps, args.warmup, seconds_per_step=8.0)
+    wl, label = workload_for(args.config)
+    if args.config == 5:
+        wl = wl.patch_workload(0)
+    value, s_per_step, cores, sample = run_oracle_steps(wl, label, args.steps, args.warmup, seconds_per_step=5.0)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": s_per_step * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "impl": "reference",
-            "config": {"workload": "config2 (BASELINE.json configs[1]), bounded sub-grid", "sample": sample},
+            "config": {"workload": f"{label}, bounded sub-grid", "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -171,6 +196,22 @@ def main_reference(args, rank, world):
 # ---------------------------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------------------------
+class Patch:
+    """One sky patch resident on the device + the step of the hot path over it."""
+
+    def __init__(self, torch, bsh, ctx, wl):
+        self.torch, self.bsh, self.ctx, self.wl = torch, bsh, ctx, wl
+        self.d_rho = torch.from_numpy(wl.rho).cuda()
+        self.d_w = torch.from_numpy(wl.w).cuda()
+
+    def step(self, mode, topk=None):
+        ctx, wl = self.ctx, self.wl
+        d_peak = ctx.build_peakgram(self.d_rho, 1.6)
+        d_top, n_top = ctx.stage1_hough(d_peak, wl, mode=mode, topk=topk or wl.topk, d_w=self.d_w)
+        ctx.stage2_power(self.d_rho, wl, d_top, n_top, d_w=self.d_w, sort_by_power=True)
+        return d_top, n_top
+
+
 def main_ours(args, rank, local_rank, world):
     import torch
     import paper_1904_04873_b200 as bsh
@@ -185,23 +226,10 @@ def main_ours(args, rank, local_rank, world):
         dist = dist_mod
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    wl = synth.config2(seed=2 + rank)                      # each rank owns a different seeded patch (weak scaling)
     ctx = bsh.Context(local_rank)
-    d_rho = torch.from_numpy(wl.rho).cuda()
-    d_w = torch.from_numpy(wl.w).cuda()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
-    h_rho = torch.from_numpy(wl.rho).pin_memory()
-    h_w = torch.from_numpy(wl.w).pin_memory()
-    h_out = torch.zeros(wl.topk * bsh.CAND_DTYPE.itemsize, dtype=torch.uint8).pin_memory()
-    h_out_np = h_out.numpy().view(bsh.CAND_DTYPE)
 
-    def step(mode):
-        d_peak = ctx.build_peakgram(d_rho, 1.6)
-        d_top, n_top = ctx.stage1_hough(d_peak, wl, mode=mode, topk=wl.topk, d_w=d_w)
-        ctx.stage2_power(d_rho, wl, d_top, n_top, d_w=d_w, sort_by_power=True)
-        return d_top, n_top
-
-    def timed(fn, steps, warmup):
+    def timed(fn, steps, warmup, stat_key="stage1_kernel_ms"):
         for _ in range(warmup):
             fn()
         torch.cuda.synchronize()
@@ -218,7 +246,7 @@ def main_ours(args, rank, local_rank, world):
             fn()
             b.record()
             b.synchronize()
-            kern_ms.append(ctx.stats()["stage1_kernel_ms"])
+            kern_ms.append(ctx.stats()[stat_key])
         torch.cuda.synchronize()
         wall = time.perf_counter() - t0
         if dist:
@@ -226,119 +254,281 @@ def main_ours(args, rank, local_rank, world):
         total_ms = sum(a.elapsed_time(b) for a, b in ev)
         launches = ctx.stats()["launches"] - l0
         total_ms = sharding.max_over_ranks(total_ms, dist)
-        return total_ms, kern_ms, launches, wall
+        return total_ms, float(np.mean(kern_ms)), launches, wall
+
+    peaks = ctx.measure_peaks() if rank == 0 else None
+
+    if args.config == 5:
+        return main_config5(args, rank, world, torch, bsh, ctx, dist, peaks)
+
+    wl, label = workload_for(args.config, rank)              # each rank owns a different seeded patch (weak scaling)
+    patch = Patch(torch, bsh, ctx, wl)
+    head_mode = bsh.BSH_WEIGHTED if args.config == 3 else bsh.BSH_UNWEIGHTED
+    other_mode = bsh.BSH_UNWEIGHTED if args.config == 3 else bsh.BSH_WEIGHTED
+    names = {bsh.BSH_WEIGHTED: "weighted", bsh.BSH_UNWEIGHTED: "unweighted"}
+
+    if args.profile:                                         # the command ncu wraps: only the chosen accumulation mode
+        mode = bsh.BSH_WEIGHTED if args.profile == "weighted" else bsh.BSH_UNWEIGHTED
+        _, k_ms, _, _ = timed(lambda: patch.step(mode), args.steps, args.warmup)
+        print(json.dumps({"profile_run": True, "config": args.config, "mode": args.profile, "kernel_ms": k_ms}), flush=True)
+        return
 
     sampler = ClockSampler(physical_gpu_index(local_rank))
     sampler.start()
-    total_ms, kern_ms, launches, wall = timed(lambda: step(bsh.BSH_UNWEIGHTED), args.steps, args.warmup)
+    total_ms, k_ms, launches, wall = timed(lambda: patch.step(head_mode), args.steps, args.warmup)
     clocks = sampler.result()
     st = ctx.stats()
     acc_per_step = wl.n_accumulations
     value = world * args.steps * acc_per_step / (total_ms * 1e-3)
 
-    # secondary: the weighted number count (FP32 weighted sum) on the same patch
-    w_steps = max(1, min(args.steps, 5))
-    if args.no_weighted:
-        print(json.dumps({"profile_run": True, "unweighted_kernel_ms": float(np.mean(kern_ms))}), flush=True)
-        return
-    w_total_ms, w_kern_ms, _, _ = timed(lambda: step(bsh.BSH_WEIGHTED), w_steps, 1)
-    st_w = ctx.stats()
-
-    if args.profile:
-        print(json.dumps({"profile_run": True, "unweighted_kernel_ms": float(np.mean(kern_ms)),
-                          "weighted_kernel_ms": float(np.mean(w_kern_ms))}), flush=True)
-        return
+    # the other number count on the same patch
+    o_steps = max(1, min(args.steps, 5))
+    o_total_ms, ok_ms, _, _ = timed(lambda: patch.step(other_mode), o_steps, 1)
+    st_o = ctx.stats()
 
     # end to end through the host-buffer entry point
+    h_rho = torch.from_numpy(wl.rho).pin_memory()
+    h_w = torch.from_numpy(wl.w).pin_memory()
+    h_out = torch.zeros(wl.topk * bsh.CAND_DTYPE.itemsize, dtype=torch.uint8).pin_memory()
+    h_out_np = h_out.numpy().view(bsh.CAND_DTYPE)
+
     def e2e_step():
-        ctx.search_patch_host(h_rho.numpy(), h_w.numpy(), wl, mode=bsh.BSH_UNWEIGHTED, topk=wl.topk, out=h_out_np)
-    e_total_ms, _, _, e_wall = timed(e2e_step, args.steps, max(1, min(args.warmup, 2)))
-    e2e_value = world * args.steps * acc_per_step / (total_ms_safe(e_total_ms))
+        ctx.search_patch_host(h_rho.numpy(), h_w.numpy(), wl, mode=head_mode, topk=wl.topk, out=h_out_np)
+    e_steps = max(1, min(args.steps, 10))
+    e_total_ms, _, _, _ = timed(e2e_step, e_steps, max(1, min(args.warmup, 2)))
+    e2e_value = world * e_steps * acc_per_step / (max(e_total_ms, 1e-9) * 1e-3)
 
     if rank != 0:
         if dist:
             dist.destroy_process_group()
         return
 
-    peaks = measured_peaks()
-    sm_max = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
-    k_ms = float(np.mean(kern_ms))
-    triples = wl.n_pix * wl.n_binary * wl.n_sft
-    issue_peak = N_SM * LANES_PER_SM_CLK * sm_max * 1e6 / 1e12                    # Tlaneop/s
-    smem_peak = N_SM * SMEM_BYTES_PER_CLK_SM * sm_max * 1e6 / 1e9                 # GB/s
-    smem_achieved = triples * SMEM_BYTES_PER_TRIPLE / (k_ms * 1e-3) / 1e9
-    alu_peak = N_SM * ALU_LANES_PER_SM_CLK * sm_max * 1e6 / 1e12
-    alu_achieved = triples * ALU_OPS_PER_TRIPLE / (k_ms * 1e-3) / 1e12
-    algo_achieved = triples * ALGO_OPS_PER_TRIPLE / (k_ms * 1e-3) / 1e12
-    gather_peak = N_SM * GATHER_LANES_PER_SM_CLK * sm_max * 1e6
-    wk_ms = float(np.mean(w_kern_ms))
-    w_ops = triples * OPS_PER_TRIPLE_WEIGHTED_FIXED + wl.n_accumulations * OPS_PER_ACC_WEIGHTED
-    cpu_value, _, cores, sample = run_oracle_steps(wl, 1, 0, seconds_per_step=15.0)
-    kname = {2: "stage1_unweighted_pix_kernel", 1: "stage1_unweighted_pos_kernel"}.get(st["kernel_variant"] // 1000,
-                                                                                       "stage1_unweighted_kernel")
+    extras = {}
+    if args.config == 3 and not args.lean:
+        extras["config2"] = sub_config2(torch, bsh, ctx, timed, peaks)
+        extras["config5_sweep"] = sweep_config5(torch, bsh, n_patches=32)
+        extras["nc_fraction"] = sub_nc_fraction(torch, bsh, ctx)
 
+    kinds = {names[head_mode]: (k_ms, total_ms / args.steps, st), names[other_mode]: (ok_ms, o_total_ms / o_steps, st_o)}
+    roof = {m: roofline(m, wl, kinds[m][0], kinds[m][2], peaks) for m in kinds}
+    head = names[head_mode]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64 track / u32 bit-sliced count / f32 power", "data": "synthetic",
-        "config": {"workload": "config2 (BASELINE.json configs[1]): 1 sky patch, 2000 SFTs, 8x8 pixels, 20x30x40 binary "
-                               "templates, 90 f0 bins; unweighted number count -> top-1000 -> stage-2 power",
+        "dtype": ("f64 track / f32 weighted count / f32 power" if head == "weighted"
+                  else "f64 track / u32 bit-sliced count / f32 power"),
+        "data": "synthetic",
+        "config": {"workload": f"{label}: 1 sky patch, {wl.n_sft} SFTs, {wl.n_pix} pixels, {len(wl.ap)}x{len(wl.P)}x"
+                               f"{len(wl.tasc_frac)} binary templates, {wl.n_f0} f0 bins; {head} number count -> top-"
+                               f"{wl.topk} -> stage-2 power",
                    "templates_per_patch": wl.n_templates, "accumulations_per_patch": acc_per_step,
                    "l2": "256 MiB buffer written between timed iterations", "ms_per_sky_patch": total_ms / args.steps,
                    "patches_per_rank": 1},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(wl.rho.nbytes + wl.w.nbytes),
-                "d2h_bytes_per_step": int(h_out.numel()), "ms_per_step": e_total_ms / args.steps,
+                "d2h_bytes_per_step": int(h_out.numel()), "ms_per_step": e_total_ms / e_steps, "steps": e_steps,
                 "call": "bsh_search_patch_host (pinned host buffers)"},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "alu", "kernel": kname, "achieved": algo_achieved, "peak": issue_peak, "unit": "Tlaneop/s",
-                     "frac": algo_achieved / issue_peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
-                     "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (total_ms / args.steps),
-                     "ops_per_triple": ALGO_OPS_PER_TRIPLE, "triples_per_launch": triples,
-                     "peak_source": f"warp-issue peak: 148 SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz (guide unit counts "
-                                    "and clock; MEASURED_PEAKS.json holds only HBM and bf16 peaks, and HBM is idle here: "
-                                    "13.5 MB of DRAM traffic per launch)",
-                     "smem_view": {"bytes_per_triple": SMEM_BYTES_PER_TRIPLE, "achieved_gbs": smem_achieved,
-                                   "peak_gbs": smem_peak, "frac": smem_achieved / smem_peak},
-                     "alu_pipe_view": {"ops_per_triple": ALU_OPS_PER_TRIPLE, "achieved_tlaneops": alu_achieved,
-                                       "peak_tlaneops": alu_peak, "frac": alu_achieved / alu_peak},
-                     "gather_bound": {"note": "north_star bound (b) read literally: one 4-byte shared-memory lane-gather "
-                                              "per accumulation at 32 lanes/clk/SM; > 1 because the 90 f0 bins of a band "
-                                              "share each gathered window",
-                                      "achieved_gathers_per_s": acc_per_step / (k_ms * 1e-3), "peak": gather_peak,
-                                      "frac": acc_per_step / (k_ms * 1e-3) / gather_peak},
-                     "hbm_bound": {"note": "position table + (cos, sin) + D tables are ~3 MB per patch, read once from "
-                                           "DRAM then served by L2: ~0.5 us at the measured HBM rate, never the bound",
-                                   "hbm_gbs_measured": peaks.get("hbm_gbs")}},
-        "weighted": {"value": world * w_steps * acc_per_step / (w_total_ms * 1e-3), "unit": UNIT,
-                     "ms_per_step": w_total_ms / w_steps, "kernel_ms": wk_ms, "kernel": "stage1_weighted_kernel",
-                     "roofline_frac_issue": w_ops / (wk_ms * 1e-3) / 1e12 / issue_peak, "n_passes": st_w["n_passes"]},
+        "roofline": roof[head],
+        names[other_mode]: {"value": world * o_steps * acc_per_step / (o_total_ms * 1e-3), "unit": UNIT,
+                            "ms_per_step": o_total_ms / o_steps, "steps": o_steps, "roofline": roof[names[other_mode]],
+                            "n_passes": st_o["n_passes"]},
         "stage_ms": {"peakgram": st["peakgram_ms"], "stage1_setup": st["stage1_setup_ms"], "stage1_kernel": k_ms,
                      "stage1_select": st["stage1_select_ms"], "stage2": st["stage2_ms"]},
         "stage1": {"n_candidates": st["n_candidates"], "threshold": st["threshold"], "n_passes": st["n_passes"],
                    "kernel_variant": st["kernel_variant"], "threads_per_block": st["threads_per_block"],
                    "grid_blocks": st["grid_blocks"]},
-        "cpu_baseline": {"value": cpu_value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "measured_peaks": peaks,
+        "cpu_baseline": cpu_baseline(wl, label),
         "wall_s_timed_region": wall,
     }
+    line.update(extras)
     print(json.dumps(line), flush=True)
     if dist:
         dist.destroy_process_group()
 
 
-def total_ms_safe(ms):
-    return max(ms, 1e-9) * 1e-3
+def kernel_name(variant: int, weighted: bool) -> str:
+    fam = variant // 1000
+    if weighted:
+        return {2: "stage1_weighted_pix_kernel", 1: "stage1_weighted_pos_kernel"}.get(fam, "stage1_weighted_kernel")
+    return {2: "stage1_unweighted_pix_kernel", 1: "stage1_unweighted_pos_kernel"}.get(fam, "stage1_unweighted_kernel")
+
+
+def roofline(mode: str, wl, k_ms: float, st: dict, pk: dict) -> dict:
+    """Roofline object of the stage-1 accumulation kernel of `mode` against the peaks measured in this run."""
+    n_sm, mhz = pk["n_sm"], pk["sm_clock_mhz"]
+    per_s = n_sm * mhz * 1e6                                          # SM-clocks per second, whole chip
+    triples = wl.n_pix * wl.n_binary * wl.n_sft
+    acc = wl.n_accumulations
+    secs = k_ms * 1e-3
+    common = {"kernel": kernel_name(st["kernel_variant"], mode == "weighted"), "kernel_ms": k_ms,
+              "traffic": NCU_DRAM_BYTES[mode], "traffic_source": NCU_DRAM_SOURCE,
+              "gather_bound": {"note": "north_star bound (b) read literally: one 4-byte shared-memory lane-gather per "
+                                       "accumulation at 32 lanes/clk/SM; the 90 f0 bins of a band share each gathered window",
+                               "frac": acc / secs / (GATHER_LANES_PER_SM_CLK * per_s)},
+              "hbm_bound": {"note": "tables of a patch are a few MB, read once from DRAM then served by L2: never the bound",
+                            "hbm_gbs_measured": measured_peaks_file().get("hbm_gbs")}}
+    if mode == "weighted":
+        peak = pk["fadd_lanes_per_clk_sm"] * per_s / 1e12
+        achieved = acc / secs / 1e12
+        return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFADD/s (one FP32 add per accumulation)",
+                "frac": achieved / peak, "ops_per_accumulation": 1.0, "accumulations_per_launch_set": acc,
+                "peak_source": f"measured in this run (bsh_measure_peaks): predicated FADD {pk['fadd_lanes_per_clk_sm']:.1f} "
+                               f"lanes/clk/SM x {n_sm} SMs x {mhz:.0f} MHz", **common}
+    issue_lanes = 128.0 * pk["issue_warp_inst_per_clk_smsp"]
+    peak = issue_lanes * per_s / 1e12
+    achieved = triples * ALGO_OPS_PER_TRIPLE / secs / 1e12
+    lds_peak = pk["lds64_bytes_per_clk_sm"] * per_s / 1e9
+    lds_ach = triples * SMEM_BYTES_PER_TRIPLE / secs / 1e9
+    alu_peak = pk["lop3_lanes_per_clk_sm"] * per_s / 1e12
+    alu_ach = triples * ALU_OPS_PER_TRIPLE / secs / 1e12
+    fp64_peak = min(pk["dadd_lanes_per_clk_sm"], pk["dmul_lanes_per_clk_sm"]) * per_s / 1e12
+    return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlaneop/s", "frac": achieved / peak,
+            "ops_per_triple": ALGO_OPS_PER_TRIPLE, "triples_per_launch": triples,
+            "peak_source": f"measured in this run (bsh_measure_peaks): warp-issue rate {pk['issue_warp_inst_per_clk_smsp']:.3f} "
+                           f"warp-instructions/clk/scheduler x 4 x 32 lanes x {n_sm} SMs x {mhz:.0f} MHz",
+            "smem_view": {"bytes_per_triple": SMEM_BYTES_PER_TRIPLE, "achieved_gbs": lds_ach, "peak_gbs": lds_peak,
+                          "frac": lds_ach / lds_peak, "peak_source": "measured conflict-free LDS.64"},
+            "alu_pipe_view": {"ops_per_triple": ALU_OPS_PER_TRIPLE, "achieved_tlaneops": alu_ach, "peak_tlaneops": alu_peak,
+                              "frac": alu_ach / alu_peak, "peak_source": "measured LOP3"},
+            "fp64_pipe_view": {"ops_per_triple": 6.0, "achieved_tlaneops": triples * 6.0 / secs / 1e12,
+                               "peak_tlaneops": fp64_peak, "frac": triples * 6.0 / secs / 1e12 / fp64_peak,
+                               "peak_source": "measured DADD / DMUL (no FMA)"},
+            **common}
+
+
+def sub_config2(torch, bsh, ctx, timed, peaks):
+    wl = synth.config2()
+    patch = Patch(torch, bsh, ctx, wl)
+    out = {"workload": "config2 (BASELINE.json configs[1]): 2000 SFTs, 1.3824e8 templates", "accumulations_per_patch": wl.n_accumulations}
+    for mode, name, steps in ((bsh.BSH_UNWEIGHTED, "unweighted", 10), (bsh.BSH_WEIGHTED, "weighted", 5)):
+        total_ms, k_ms, _, _ = timed(lambda: patch.step(mode), steps, 3)
+        st = ctx.stats()
+        out[name] = {"value": steps * wl.n_accumulations / (total_ms * 1e-3), "unit": UNIT, "ms_per_step": total_ms / steps,
+                     "steps": steps, "roofline": roofline(name, wl, k_ms, st, peaks)}
+    return out
+
+
+def sweep_config5(torch, bsh, n_patches=32, c5=None):
+    """Config 5: patches of the hemisphere tiling streamed over two CUDA streams (two contexts), one shared peakgram;
+    the launch/collect split lets patch n + 1 accumulate while patch n is selected and re-scored.  Device-timed: events
+    on both streams, max of the two."""
+    c5 = c5 or synth.config5()
+    stride = max(1, c5.n_patches // n_patches)
+    ids = [i * stride for i in range(n_patches)]              # spread over the whole hemisphere (all declinations)
+    wls = [c5.patch_workload(i) for i in ids]
+    d_rho = torch.from_numpy(c5.base.rho).cuda()
+    out = {"workload": f"config5 (BASELINE.json configs[4]): {n_patches} of the 256 patches (every {stride}th), 8000 SFTs, "
+                       "1.3824e8 templates per patch, unweighted count -> top-1000 -> stage 2 per patch",
+           "patches": n_patches}
+    for n_streams in (1, 2):
+        streams = [torch.cuda.Stream() for _ in range(n_streams)]
+        ctxs = [bsh.Context(0, stream=s) for s in streams]
+        with torch.cuda.stream(streams[0]):
+            d_peak = ctxs[0].build_peakgram(d_rho)
+        torch.cuda.synchronize()
+        keep = [torch.from_numpy(w.w).cuda() for w in wls]
+        for rep in range(2):                                  # first pass warms tables and allocations
+            torch.cuda.synchronize()
+            start = [torch.cuda.Event(enable_timing=True) for _ in streams]
+            stop = [torch.cuda.Event(enable_timing=True) for _ in streams]
+            for s, e in zip(streams, start):
+                e.record(s)
+            t0 = time.perf_counter()
+            pending = [None] * n_streams
+            for n, ip in enumerate(list(range(n_patches)) + [None] * n_streams):
+                s = n % n_streams
+                if pending[s] is not None:
+                    jp = pending[s]
+                    with torch.cuda.stream(streams[s]):
+                        d_top, n_top = ctxs[s].stage1_collect()
+                        ctxs[s].stage2_power(d_rho, wls[jp], d_top, n_top, d_w=keep[jp], sort_by_power=True)
+                    pending[s] = None
+                if ip is not None:
+                    with torch.cuda.stream(streams[s]):
+                        ctxs[s].stage1_launch(d_peak, wls[ip], mode=bsh.BSH_UNWEIGHTED, topk=1000, d_w=keep[ip])
+                    pending[s] = ip
+            for s, e in zip(streams, stop):
+                e.record(s)
+            torch.cuda.synchronize()
+            wall = time.perf_counter() - t0
+            dev_ms = max(a.elapsed_time(b) for a in start for b in stop)
+        acc = sum(w.n_accumulations for w in wls)
+        out[f"streams_{n_streams}"] = {"ms_per_patch": dev_ms / n_patches, "value": acc / (dev_ms * 1e-3), "unit": UNIT,
+                                      "wall_ms_per_patch": wall / n_patches * 1e3}
+        for c in ctxs:
+            c.close()
+    return out
+
+
+def sub_nc_fraction(torch, bsh, ctx):
+    """toplist = fraction N_C = 5 % of config 2's templates, stage 2 on the
+    half-overlapped SFT set (2 N rows)."""
+    wl = synth.config2()
+    wl2 = synth.overlapped_stage2_set(wl, seed=12)
+    k = int(0.05 * wl.n_templates)
+    d_rho, d_w = torch.from_numpy(wl.rho).cuda(), torch.from_numpy(wl.w).cuda()
+    d_rho2, d_w2 = torch.from_numpy(wl2.rho).cuda(), torch.from_numpy(wl2.w).cuda()
+    res = {}
+    for rep in range(2):
+        torch.cuda.synchronize()
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        e[0].record()
+        d_peak = ctx.build_peakgram(d_rho, 1.6)
+        d_top, n_top = ctx.stage1_hough(d_peak, wl, mode=bsh.BSH_UNWEIGHTED, topk=k, d_w=d_w)
+        e[1].record()
+        ctx.stage2_power(d_rho2, wl2, d_top, n_top, d_w=d_w2, sort_by_power=True)
+        e[2].record()
+        torch.cuda.synchronize()
+        st = ctx.stats()
+        res = {"workload": "config 2, N_C = 5 % of 1.3824e8 templates -> stage 2 on 4000 half-overlapped SFTs",
+               "candidates": n_top, "stage1_ms": e[0].elapsed_time(e[1]), "selection_ms": st["stage1_select_ms"],
+               "stage2_ms": e[1].elapsed_time(e[2]), "total_ms": e[0].elapsed_time(e[2]),
+               "stage2_gathers_per_s": n_top * wl2.n_sft / (e[1].elapsed_time(e[2]) * 1e-3),
+               "n_passes": st["n_passes"]}
+        del d_top
+    return res
+
+
+def main_config5(args, rank, world, torch, bsh, ctx, dist, peaks):
+    c5, label = workload_for(5, rank)
+    n_patches = max(2, args.steps)
+    sampler = ClockSampler(physical_gpu_index(int(os.environ.get("LOCAL_RANK", "0"))))
+    sampler.start()
+    sw = sweep_config5(torch, bsh, n_patches=n_patches, c5=c5)
+    clocks = sampler.result()
+    if dist:
+        dist.barrier()
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+    two = sw["streams_2"]
+    wl0 = c5.patch_workload(0)
+    line = {"metric": METRIC, "value": world * two["value"], "unit": UNIT, "n_gpus": world, "steps": n_patches,
+            "warmup": n_patches, "ms_per_step": two["ms_per_patch"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64 track / u32 bit-sliced count / f32 power", "data": "synthetic",
+            "config": {"workload": sw["workload"], "ms_per_sky_patch": two["ms_per_patch"],
+                       "l2": "per-patch tables exceed nothing; patches differ, 8 MB power slab re-read per patch",
+                       "templates_per_patch": wl0.n_templates, "accumulations_per_patch": wl0.n_accumulations},
+            "clocks": clocks, "sweep": sw, "measured_peaks": peaks, "gpu_launches": None,
+            "note": "a step is one sky patch; the first sweep over the patches is the warm-up"}
+    print(json.dumps(line), flush=True)
+    if dist:
+        dist.destroy_process_group()
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[2, 3, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--profile", action="store_true",
-                    help="only the timed unweighted + weighted steps (no e2e, no oracle): the command ncu wraps")
-    ap.add_argument("--no-weighted", action="store_true", help="with --profile: skip the weighted-count pass")
+    ap.add_argument("--lean", action="store_true", help="skip the config-2 / config-5 / N_C sub-objects of the default line")
+    ap.add_argument("--profile", default=None, choices=["weighted", "unweighted"],
+                    help="only the timed steps of one accumulation mode (no e2e, no oracle): the command ncu wraps")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

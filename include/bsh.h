@@ -44,6 +44,16 @@ extern "C" {
 #define BSH_NAIVE      16 /* diagnostic: one thread per template, one track evaluation per (template, SFT), global-
                              memory gathers.  Same results; exists to cross-check the tiled kernels at full size. */
 
+/* bsh_set_option(): DIAGNOSTIC switches, so that the tests can reach every kernel family and both table geometries
+ * on any input.  Production leaves the defaults (the library picks the family from the problem shape). */
+#define BSH_OPT_KERNEL_FAMILY      1   /* one of BSH_FAMILY_*                                                      */
+#define BSH_OPT_FORCE_CLAMP        2   /* 1: use the clamped table geometry even when no track can leave the slab  */
+#define BSH_OPT_PIXELS_PER_THREAD  3   /* window-table family only: 0 = auto, 1, 2                                 */
+#define BSH_FAMILY_AUTO        0
+#define BSH_FAMILY_PIXEL_LANE  1       /* sky pixels on the lanes (bsh_pix.cuh)                                    */
+#define BSH_FAMILY_TEMPLATE_LANE 2     /* binary templates on the lanes, position table (bsh_pos.cuh)              */
+#define BSH_FAMILY_WINDOW      3       /* binary templates on the lanes, funnel-shift window table (wide slabs)    */
+
 typedef struct bsh_ctx bsh_ctx;
 
 /* One SFT set.  Stage 1 and stage 2 may be given different sets (the paper's stage 2 adds half-overlapped SFTs,
@@ -99,6 +109,23 @@ typedef struct {
     float    host_tables_ms;     /* host time spent building cos/sin tables in the last call (0 when cached)       */
 } bsh_stats;
 
+/* On-chip peak rates of the context's device, MEASURED by bsh_measure_peaks() with microbenchmark kernels (32 warps
+ * per SM on every SM, volatile inline PTX, timed with clock64 per block).  They are the denominators of
+ * the roofline fractions of the stage-1 accumulation kernels, which are bound on chip and not by HBM. */
+typedef struct {
+    int32_t n_sm;                          /* multiprocessors                                                     */
+    double  sm_clock_mhz;                  /* SM clock during the measurement (clock64 against globaltimer)       */
+    double  issue_warp_inst_per_clk_smsp;  /* alternating LOP3 / FADD stream: warp instructions per clock per     */
+                                           /*   scheduler (SM sub-partition); lanes/clk/SM = 128 x this           */
+    double  lop3_lanes_per_clk_sm;         /* integer-ALU pipe (bit-sliced counters)                              */
+    double  fadd_lanes_per_clk_sm;         /* predicated FP32 add (weighted number count, L223)                   */
+    double  dadd_lanes_per_clk_sm;         /* FP64 add, no FMA (canonical track, R-5)                             */
+    double  dmul_lanes_per_clk_sm;         /* FP64 multiply                                                       */
+    double  lds32_bytes_per_clk_sm;        /* conflict-free shared-memory loads: LDS.32 / LDS.64 / LDS.128        */
+    double  lds64_bytes_per_clk_sm;
+    double  lds128_bytes_per_clk_sm;
+} bsh_peaks;
+
 /* Create a context bound to `device` and to `cuda_stream` (a cudaStream_t; NULL = legacy default stream).
  * The context owns scratch memory (tables, candidate buffer), grown on demand and freed by bsh_destroy. */
 int bsh_create(bsh_ctx **out, int device, void *cuda_stream);
@@ -106,6 +133,8 @@ int bsh_destroy(bsh_ctx *ctx);
 const char *bsh_last_error(const bsh_ctx *ctx);
 int bsh_get_stats(bsh_ctx *ctx, bsh_stats *out);     /* synchronises the stream to read event timers */
 int bsh_version(void);
+int bsh_set_option(bsh_ctx *ctx, int32_t option, int32_t value);   /* BSH_EINVAL for an unknown option / value      */
+int bsh_measure_peaks(bsh_ctx *ctx, bsh_peaks *h_out);             /* ~50 ms of device time; synchronous            */
 
 /* Peakgram (L176): d_peak[i][k >> 5] bit (k & 31) = (d_rho[i * rho_row_stride + k] > rho_th), strict '>' in FP32,
  * NaN -> 0 (R-8); pad bits of each row are zero.  d_rho: [n_sft][rho_row_stride] FP32, rho_row_stride >= n_bins

@@ -10,8 +10,11 @@ import numpy as np
 from . import build as _build
 
 BSH_UNWEIGHTED, BSH_WEIGHTED, BSH_NAIVE = 0, 1, 16
+BSH_OPT_KERNEL_FAMILY, BSH_OPT_FORCE_CLAMP, BSH_OPT_PIXELS_PER_THREAD = 1, 2, 3
+BSH_FAMILY_AUTO, BSH_FAMILY_PIXEL_LANE, BSH_FAMILY_TEMPLATE_LANE, BSH_FAMILY_WINDOW = 0, 1, 2, 3
 
-EXPORTS = ["bsh_version", "bsh_create", "bsh_destroy", "bsh_last_error", "bsh_get_stats", "bsh_build_peakgram",
+EXPORTS = ["bsh_version", "bsh_create", "bsh_destroy", "bsh_last_error", "bsh_get_stats", "bsh_set_option",
+           "bsh_measure_peaks", "bsh_build_peakgram",
            "bsh_stage1_hough", "bsh_stage1_launch", "bsh_stage1_collect", "bsh_stage2_power", "bsh_search_patch_host",
            "bsh_template_index", "bsh_template_decode"]
 
@@ -40,6 +43,17 @@ class Stats(C.Structure):
                 ("n_accumulations", C.c_int64), ("n_candidates", C.c_int64), ("threshold", C.c_double),
                 ("n_passes", C.c_int32), ("kernel_variant", C.c_int32), ("threads_per_block", C.c_int32),
                 ("grid_blocks", C.c_int32), ("launches", C.c_int64), ("host_tables_ms", C.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class Peaks(C.Structure):
+    _fields_ = [("n_sm", C.c_int32), ("sm_clock_mhz", C.c_double), ("issue_warp_inst_per_clk_smsp", C.c_double),
+                ("lop3_lanes_per_clk_sm", C.c_double), ("fadd_lanes_per_clk_sm", C.c_double),
+                ("dadd_lanes_per_clk_sm", C.c_double), ("dmul_lanes_per_clk_sm", C.c_double),
+                ("lds32_bytes_per_clk_sm", C.c_double), ("lds64_bytes_per_clk_sm", C.c_double),
+                ("lds128_bytes_per_clk_sm", C.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -150,7 +164,8 @@ class Context:
     def stage1_collect(self):
         torch = self.torch
         pb, topk = self._pending
-        d_top = torch.empty(topk * CAND_DTYPE.itemsize, dtype=torch.uint8, device=f"cuda:{self.device}")
+        with torch.cuda.stream(self.stream):             # the records are written on the context's stream
+            d_top = torch.empty(topk * CAND_DTYPE.itemsize, dtype=torch.uint8, device=f"cuda:{self.device}")
         n_top = C.c_int32(0)
         self._check(self.lib.bsh_stage1_collect(self._ctx, C.c_void_p(d_top.data_ptr()), C.byref(n_top)))
         return d_top, int(n_top.value)
@@ -188,6 +203,16 @@ class Context:
                                                    C.byref(pb.sfts), C.byref(pb.grid), C.c_int32(mode), C.c_int32(topk),
                                                    C.c_void_p(out.ctypes.data), C.byref(n_top)))
         return out, int(n_top.value)
+
+    def set_option(self, option: int, value: int):
+        """Diagnostic switches (kernel family, table geometry); see include/bsh.h."""
+        self._check(self.lib.bsh_set_option(self._ctx, C.c_int32(option), C.c_int32(value)))
+
+    def measure_peaks(self) -> dict:
+        """Measured on-chip peak rates of this device (bsh_measure_peaks)."""
+        pk = Peaks()
+        self._check(self.lib.bsh_measure_peaks(self._ctx, C.byref(pk)))
+        return pk.as_dict()
 
     def stats(self) -> dict:
         s = Stats()

@@ -10,7 +10,8 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbsh.so")
 SOURCES = [os.path.join(CSRC, "bsh_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "bsh_kernels.cuh"), os.path.join(CSRC, "bsh_core.cuh"),
-                  os.path.join(CSRC, "bsh_pos.cuh"), os.path.join(CSRC, "bsh_pix.cuh"), os.path.join(CSRC, "bsh_host.hpp"),
+                  os.path.join(CSRC, "bsh_pos.cuh"), os.path.join(CSRC, "bsh_pix.cuh"), os.path.join(CSRC, "bsh_peaks.cuh"),
+                  os.path.join(CSRC, "bsh_host.hpp"),
                   os.path.join(HERE, "..", "include", "bsh.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -17,6 +17,7 @@
 #include "bsh_kernels.cuh"
 #include "bsh_pos.cuh"
 #include "bsh_pix.cuh"
+#include "bsh_peaks.cuh"
 
 using namespace bsh;
 
@@ -77,6 +78,8 @@ struct bsh_ctx {
     unsigned int *pinned_count = nullptr;
     cudaEvent_t ev[10] = {};
     Pending pend;
+    int opt_family = BSH_FAMILY_AUTO, opt_force_clamp = 0, opt_pixels_per_thread = 0;   // bsh_set_option
+    DevBuf peak_samples;
     bsh_stats st = {};
     bool have_pk = false, have_setup = false, have_kernel = false, have_select = false, have_s2 = false;
     float kernel_ms_extra = 0.f;
@@ -117,6 +120,22 @@ int ensure(bsh_ctx *ctx, DevBuf &b, size_t bytes)
     b.bytes = want;
     return BSH_OK;
 }
+
+// the ABI calls run on the context's device and leave the caller's current device as they found it
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != dev) cudaSetDevice(dev);
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+};
 
 #define TRY(expr)                  \
     do {                           \
@@ -167,7 +186,8 @@ int get_tables(bsh_ctx *ctx, const bsh_sfts *s, const bsh_grid *g, int *slot_out
         }
     }
     const auto t0 = std::chrono::steady_clock::now();
-    const int k = (!ctx->cache[0].valid || (ctx->cache[1].valid && ctx->cache[0].stamp < ctx->cache[1].stamp)) ? 0 : 1;
+    int k = (!ctx->cache[0].valid || (ctx->cache[1].valid && ctx->cache[0].stamp < ctx->cache[1].stamp)) ? 0 : 1;
+    if (ctx->pend.active && ctx->pend.cache_slot == k) k ^= 1;     // a launched, uncollected stage 1 still reads its slot
     TableCache &c = ctx->cache[k];
     c.valid = false;
     const int n_pad = pad_sfts(N);
@@ -473,12 +493,40 @@ int sort_candidates(bsh_ctx *ctx, RawCand *buf, unsigned int n)
 
 }  // namespace
 
+namespace {
+
+template <int OP>
+int run_peak(bsh_ctx *ctx, int n_sm, int iters, std::vector<PeakSample> &host, double *ops_per_clk_sm, double *mhz)
+{
+    PeakSample *d = (PeakSample *)ctx->peak_samples.p;
+    uint32_t *sink = (uint32_t *)((char *)ctx->peak_samples.p + sizeof(PeakSample) * (size_t)n_sm);
+    for (int rep = 0; rep < 2; ++rep) {                  // the first launch warms the instruction cache and the clocks
+        peak_kernel<OP><<<n_sm, kPeakThreads, 0, ctx->stream>>>(iters, (uint32_t)(rep + 1), sink, d);
+        count_launch(ctx);
+    }
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(host.data(), d, sizeof(PeakSample) * (size_t)n_sm, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    std::vector<double> cyc(n_sm), f(n_sm);
+    for (int b = 0; b < n_sm; ++b) {
+        cyc[b] = (double)host[b].cycles;
+        f[b] = host[b].ns ? 1e3 * (double)host[b].cycles / (double)host[b].ns : 0.0;
+    }
+    std::sort(cyc.begin(), cyc.end());
+    std::sort(f.begin(), f.end());
+    *ops_per_clk_sm = (double)kPeakThreads * iters * kPeakUnroll / cyc[n_sm / 2];
+    if (mhz) *mhz = f[n_sm / 2];
+    return BSH_OK;
+}
+
+}  // namespace
+
 // =====================================================================================================================
 // C ABI
 // =====================================================================================================================
 extern "C" {
 
-int bsh_version(void) { return 100; }
+int bsh_version(void) { return 200; }
 
 int bsh_create(bsh_ctx **out, int device, void *cuda_stream)
 {
@@ -490,7 +538,7 @@ int bsh_create(bsh_ctx **out, int device, void *cuda_stream)
     if (!ctx) return BSH_ENOMEM;
     ctx->device = device;
     ctx->stream = (cudaStream_t)cuda_stream;
-    if (cudaSetDevice(device) != cudaSuccess) { delete ctx; return BSH_ECUDA; }
+    const DeviceGuard device_guard(device);
     for (auto &e : ctx->ev)
         if (cudaEventCreate(&e) != cudaSuccess) { delete ctx; return BSH_ECUDA; }
     if (cudaMallocHost((void **)&ctx->pinned_count, 64) != cudaSuccess) { delete ctx; return BSH_ENOMEM; }
@@ -501,10 +549,10 @@ int bsh_create(bsh_ctx **out, int device, void *cuda_stream)
 int bsh_destroy(bsh_ctx *ctx)
 {
     if (!ctx) return BSH_EINVAL;
-    cudaSetDevice(ctx->device);
+    const DeviceGuard device_guard(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf *bufs[] = {&ctx->wtab, &ctx->w_pad, &ctx->stats, &ctx->thr, &ctx->dtab, &ctx->nvec, &ctx->cand, &ctx->cand_count,
-                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->psplit, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top};
+                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->psplit, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top, &ctx->peak_samples};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto &c : ctx->cache) {
@@ -524,7 +572,7 @@ const char *bsh_last_error(const bsh_ctx *ctx) { return ctx ? ctx->err.c_str() :
 int bsh_get_stats(bsh_ctx *ctx, bsh_stats *out)
 {
     if (!ctx || !out) return BSH_EINVAL;
-    CK(cudaSetDevice(ctx->device));
+    const DeviceGuard device_guard(ctx->device);
     CK(cudaStreamSynchronize(ctx->stream));
     float ms = 0.f;
     if (ctx->have_pk && cudaEventElapsedTime(&ms, ctx->ev[8], ctx->ev[9]) == cudaSuccess) ctx->st.peakgram_ms = ms;
@@ -537,6 +585,56 @@ int bsh_get_stats(bsh_ctx *ctx, bsh_stats *out)
     return BSH_OK;
 }
 
+int bsh_set_option(bsh_ctx *ctx, int32_t option, int32_t value)
+{
+    if (!ctx) return BSH_EINVAL;
+    switch (option) {
+    case BSH_OPT_KERNEL_FAMILY:
+        if (value < BSH_FAMILY_AUTO || value > BSH_FAMILY_WINDOW) return fail(ctx, BSH_EINVAL, "unknown kernel family %d", value);
+        ctx->opt_family = value;
+        return BSH_OK;
+    case BSH_OPT_FORCE_CLAMP:
+        ctx->opt_force_clamp = value != 0;
+        return BSH_OK;
+    case BSH_OPT_PIXELS_PER_THREAD:
+        if (value < 0 || value > 2) return fail(ctx, BSH_EINVAL, "pixels per thread must be 0 (auto), 1 or 2");
+        ctx->opt_pixels_per_thread = value;
+        return BSH_OK;
+    default:
+        return fail(ctx, BSH_EINVAL, "unknown option %d", option);
+    }
+}
+
+int bsh_measure_peaks(bsh_ctx *ctx, bsh_peaks *h_out)
+{
+    if (!ctx || !h_out) return BSH_EINVAL;
+    const DeviceGuard device_guard(ctx->device);
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, ctx->device));
+    const int n_sm = prop.multiProcessorCount;
+    TRY(ensure(ctx, ctx->peak_samples, sizeof(PeakSample) * (size_t)n_sm + 64));
+    std::vector<PeakSample> host(n_sm);
+    bsh_peaks pk = {};
+    pk.n_sm = n_sm;
+    double mhz[4] = {0, 0, 0, 0}, v = 0;
+    TRY(run_peak<kOpLop3>(ctx, n_sm, 4000, host, &pk.lop3_lanes_per_clk_sm, &mhz[0]));
+    TRY(run_peak<kOpFadd>(ctx, n_sm, 4000, host, &pk.fadd_lanes_per_clk_sm, &mhz[1]));
+    TRY(run_peak<kOpDadd>(ctx, n_sm, 2000, host, &pk.dadd_lanes_per_clk_sm, &mhz[2]));
+    TRY(run_peak<kOpDmul>(ctx, n_sm, 2000, host, &pk.dmul_lanes_per_clk_sm, nullptr));
+    TRY(run_peak<kOpMixed>(ctx, n_sm, 4000, host, &v, &mhz[3]));
+    pk.issue_warp_inst_per_clk_smsp = v / 32.0 / 4.0;
+    TRY(run_peak<kOpLds32>(ctx, n_sm, 2000, host, &v, nullptr));
+    pk.lds32_bytes_per_clk_sm = 4.0 * v;
+    TRY(run_peak<kOpLds64>(ctx, n_sm, 2000, host, &v, nullptr));
+    pk.lds64_bytes_per_clk_sm = 8.0 * v;
+    TRY(run_peak<kOpLds128>(ctx, n_sm, 1000, host, &v, nullptr));
+    pk.lds128_bytes_per_clk_sm = 16.0 * v;
+    std::sort(mhz, mhz + 4);
+    pk.sm_clock_mhz = 0.5 * (mhz[1] + mhz[2]);
+    *h_out = pk;
+    return BSH_OK;
+}
+
 int bsh_build_peakgram(bsh_ctx *ctx, const float *d_rho, int32_t n_sft, int32_t n_bins, int64_t rho_row_stride,
                        float rho_th, uint32_t *d_peak, int32_t words_per_row)
 {
@@ -544,7 +642,7 @@ int bsh_build_peakgram(bsh_ctx *ctx, const float *d_rho, int32_t n_sft, int32_t 
     if (!d_rho || !d_peak || n_sft < 1 || n_bins < 1 || rho_row_stride < n_bins)
         return fail(ctx, BSH_EINVAL, "bsh_build_peakgram: bad arguments");
     if ((int64_t)words_per_row * 32 < n_bins) return fail(ctx, BSH_ESMALL, "words_per_row * 32 < n_bins");
-    CK(cudaSetDevice(ctx->device));
+    const DeviceGuard device_guard(ctx->device);
     CK(cudaEventRecord(ctx->ev[8], ctx->stream));
     const bool vec4 = (rho_row_stride % 4 == 0) && ((uintptr_t)d_rho % 16 == 0);
     if (vec4) {
@@ -573,7 +671,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     if ((int64_t)words_per_row * 32 < sfts->n_bins) return fail(ctx, BSH_ESMALL, "words_per_row * 32 < n_bins");
     if ((mode & BSH_WEIGHTED) && !sfts->d_w) return fail(ctx, BSH_EINVAL, "BSH_WEIGHTED needs sfts->d_w");
     if (mode & ~(BSH_WEIGHTED | BSH_NAIVE)) return fail(ctx, BSH_EINVAL, "unknown mode bits");
-    CK(cudaSetDevice(ctx->device));
+    const DeviceGuard device_guard(ctx->device);
     ctx->pend.active = false;
 
     Pending pd;
@@ -594,27 +692,22 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     pd.tile_bins = 32 * pd.NW;
     // weighted count: one FP32 accumulator per bin lives in registers; 90 of them spill (ncu: 0.2 local-memory accesses
     // per accumulation), so a band of 65..96 bins is done as two passes of half the bins (two-word windows)
-    if (weighted && grid->n_f0 > 64 && grid->n_f0 <= 96 && getenv("BSH_W_FULLTILE") == nullptr) {
+    if (weighted && grid->n_f0 > 64 && grid->n_f0 <= 96) {
         pd.NW = 2;
         pd.tile_bins = (grid->n_f0 + 1) / 2;
     }
-    if (const char *e = getenv("BSH_PIXELS_PER_THREAD")) {
-        const int r = atoi(e);
-        if (!weighted && (r == 1 || r == 2)) pd.R = r;
-    }
+    if (!weighted && (ctx->opt_pixels_per_thread == 1 || ctx->opt_pixels_per_thread == 2)) pd.R = ctx->opt_pixels_per_thread;
     pd.HP = sfts->n_sft < (1 << 11) ? 6 : (sfts->n_sft < (1 << 13) ? 8 : 11);
     if (sfts->n_sft >= (1 << 16)) return fail(ctx, BSH_EINVAL, "n_sft >= 65536 not supported");
     const TableGeometry tg = table_geometry(sfts->n_sft, sfts->h_v_over_c, grid->n_P, grid->h_P, grid->n_ap, grid->h_ap,
                                             grid->k_band0, sfts->k_slab0, grid->n_f0, sfts->n_bins, pd.NW,
-                                            getenv("BSH_FORCE_CLAMP") != nullptr);
+                                            ctx->opt_force_clamp != 0);
     pd.clamp = tg.clamp; pd.off_table = tg.off_table; pd.s_max = tg.s_max; pd.n_entries = tg.n_entries;
     pd.s_zero = tg.s_zero;
     const int n_aq = grid->n_ap * grid->n_tasc;
     pd.tpb = pick_threads_per_block(n_aq);
-    if (const char *e = getenv("BSH_TPB")) pd.tpb = std::max(32, std::min(256, atoi(e) / 32 * 32));
     pd.n_aq_tiles = (n_aq + pd.tpb - 1) / pd.tpb;
     pd.list_cap = 48;
-    if (const char *e = getenv("BSH_LIST_CAP")) pd.list_cap = std::max(1, atoi(e));
     pd.n_groups = (grid->n_pix + pd.R - 1) / pd.R;
     {   // position-table kernels when 2+ stages of the table fit in shared memory (else the funnel-shift kernels)
         const PosGeometry pg = pos_geometry(tg, sfts->n_bins, grid->n_f0, pd.NW, pd.tile_bins);
@@ -625,8 +718,8 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         const int budgets[3] = {112 * 1024, 112 * 1024, 224 * 1024};                          // 2 / 2 / 1 blocks per SM
         pd.n_stages = 0;
         for (int b = 0; b < 3 && pd.n_stages < 2; ++b) pd.n_stages = std::min(kMaxStages, (budgets[b] - kPosHeader) / stride);
-        if (const char *e = getenv("BSH_STAGES")) pd.n_stages = std::min(pd.n_stages, std::max(2, atoi(e)));
-        pd.use_pos = pd.n_stages >= 2 && getenv("BSH_LEGACY") == nullptr && !(mode & BSH_NAIVE);
+        const int fam = ctx->opt_family;
+        pd.use_pos = pd.n_stages >= 2 && fam != BSH_FAMILY_WINDOW && !(mode & BSH_NAIVE);
         pd.n_stages = std::min(pd.n_stages, pd.n_pad / kStageSfts);
         pd.pos_groups = weighted ? grid->n_pix : (grid->n_pix + 1) / 2;
         pd.n_oct = (pd.pos_groups + wpb - 1) / wpb;
@@ -638,13 +731,11 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         const int hi_bytes = pix_hi_bytes(pd.NW, pd.HP);                                    // shared-memory high planes
         for (int b = 1; b < 3 && pd.pix_stages < 2; ++b)
             pd.pix_stages = std::min(4, (budgets[b] - kPixHeader - hi_bytes) / ps.stride);      // (2..6 stages measure alike)
-        if (const char *e = getenv("BSH_STAGES")) pd.pix_stages = std::min(pd.pix_stages, std::max(2, atoi(e)));
         const bool lanes_ok = 10 * grid->n_pix >= 6 * 32 * pd.n_pg;
-        pd.use_pix = !weighted && pd.pix_stages >= 2 && (lanes_ok || getenv("BSH_FORCE_PIX") != nullptr) &&
-                     getenv("BSH_LEGACY") == nullptr && getenv("BSH_NO_PIX") == nullptr && !(mode & BSH_NAIVE);
+        pd.use_pix = !weighted && pd.pix_stages >= 2 && (lanes_ok || fam == BSH_FAMILY_PIXEL_LANE) &&
+                     (fam == BSH_FAMILY_AUTO || fam == BSH_FAMILY_PIXEL_LANE) && !(mode & BSH_NAIVE);
         pd.pix_stages = std::max(1, std::min(pd.pix_stages, pd.n_pad / kStageSfts));
         pd.pix_smem = kPixHeader + pd.pix_stages * ps.stride + hi_bytes;
-        if (const char *e = getenv("BSH_SMEM_PAD")) pd.pix_smem += atoi(e);              // tuning: lowers the occupancy
     }
     // Toplists as large as a fraction N_C of the bank (L225: 5-10 % of all templates go to stage 2) need a larger
     // candidate buffer and a tighter first guess of the threshold (1.3 k instead of 8 k expected survivors).
@@ -732,7 +823,7 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
     if (!ctx) return BSH_EINVAL;
     if (!ctx->pend.active) return fail(ctx, BSH_ESTATE, "bsh_stage1_collect without a pending bsh_stage1_launch");
     if (!d_top || !h_n_top) return fail(ctx, BSH_EINVAL, "null d_top / h_n_top");
-    CK(cudaSetDevice(ctx->device));
+    const DeviceGuard device_guard(ctx->device);
     Pending &pd = ctx->pend;
     const bool weighted = (pd.mode & BSH_WEIGHTED) != 0;
     const uint64_t want = std::min<uint64_t>((uint64_t)pd.topk, pd.n_templates);
@@ -764,7 +855,7 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
 
     CK(cudaEventRecord(ctx->ev[4], ctx->stream));
     RawCand *sorted = (RawCand *)ctx->cand.p;
-    if (n_cand > (unsigned)kSortTile && (uint64_t)n_cand > want && getenv("BSH_FULL_SORT") == nullptr) {
+    if (n_cand > (unsigned)kSortTile && (uint64_t)n_cand > want) {
         // only the candidates at or above the k-th largest key take part in the sort (ties at the cut included)
         TRY(ensure(ctx, ctx->keys, (size_t)pd.cand_cap * sizeof(RawCand)));
         select_cut_kernel<<<1, 1024, 0, ctx->stream>>>((const RawCand *)ctx->cand.p, n_cand, (unsigned int)want,
@@ -822,7 +913,7 @@ int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, c
     if (!d_rho || !d_cands || n_cands < 0 || rho_row_stride < sfts->n_bins)
         return fail(ctx, BSH_EINVAL, "bsh_stage2_power: bad arguments");
     if (n_cands == 0) return BSH_OK;
-    CK(cudaSetDevice(ctx->device));
+    const DeviceGuard device_guard(ctx->device);
     int slot = 0;
     TRY(get_tables(ctx, sfts, grid, &slot));
     const TableCache &c = ctx->cache[slot];
@@ -860,7 +951,7 @@ int bsh_search_patch_host(bsh_ctx *ctx, const float *h_rho, const float *h_w, fl
     TRY(validate(ctx, sfts, grid));
     if (!h_rho || !h_top || !h_n_top || topk < 1) return fail(ctx, BSH_EINVAL, "bsh_search_patch_host: bad arguments");
     if ((mode & BSH_WEIGHTED) && !h_w) return fail(ctx, BSH_EINVAL, "BSH_WEIGHTED needs h_w");
-    CK(cudaSetDevice(ctx->device));
+    const DeviceGuard device_guard(ctx->device);
     const int N = sfts->n_sft, K = sfts->n_bins, W = (K + 31) / 32;
     TRY(ensure(ctx, ctx->h_rho, sizeof(float) * (size_t)N * K));
     TRY(ensure(ctx, ctx->h_w, sizeof(float) * (size_t)N));

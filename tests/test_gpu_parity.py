@@ -167,24 +167,24 @@ def test_topk_larger_than_template_count(bsh, torch, ctx):
 @pytest.mark.parametrize("n_sft,n_f0,margin,f0,side", [(1, 1, 3, 50.0, 1), (33, 7, 12, 80.0, 1), (64, 90, 30, 120.0, 2),
                                                         (200, 96, 45, 150.0, 3), (130, 97, 45, 150.0, 2),
                                                         (70, 200, 60, 200.0, 1), (2100, 64, 50, 180.0, 1)])
-def test_ragged_sizes(bsh, torch, ctx, monkeypatch, n_sft, n_f0, margin, f0, side):
+def test_ragged_sizes(bsh, torch, ctx, n_sft, n_f0, margin, f0, side):
     wl = synth.noise_workload(seed=n_sft + n_f0, n_sft=n_sft, n_f0=n_f0, margin=margin, f_band_start=f0, n_pix_side=side,
                               ap=(10.0, 40.0), P_days=(15.0, 31.0), n_t=3, topk=7)
     pk = oracle.peakgram(wl.rho)
     want_n, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
-    for force_clamp in (False, True):
-        if force_clamp:
-            monkeypatch.setenv("BSH_FORCE_CLAMP", "1")
-        else:
-            monkeypatch.delenv("BSH_FORCE_CLAMP", raising=False)
-        for ppt in ("1", "2"):
-            monkeypatch.setenv("BSH_PIXELS_PER_THREAD", ppt)
-            r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
-            assert np.array_equal(r["counts"], want_n), (force_clamp, ppt)
-            check_unweighted_toplist(r["top"], want_n, 7)
-        r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED)
-        assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=1e-6)
-        check_float_toplist(r["top"]["index"], want_w, 7)
+    for family in (bsh.BSH_FAMILY_AUTO, bsh.BSH_FAMILY_TEMPLATE_LANE, bsh.BSH_FAMILY_WINDOW):
+        ctx.set_option(bsh.BSH_OPT_KERNEL_FAMILY, family)
+        for force_clamp in (False, True):
+            ctx.set_option(bsh.BSH_OPT_FORCE_CLAMP, int(force_clamp))
+            for ppt in ((1, 2) if family == bsh.BSH_FAMILY_WINDOW else (0,)):
+                ctx.set_option(bsh.BSH_OPT_PIXELS_PER_THREAD, ppt)
+                r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
+                assert np.array_equal(r["counts"], want_n), (family, force_clamp, ppt)
+                check_unweighted_toplist(r["top"], want_n, 7)
+            ctx.set_option(bsh.BSH_OPT_PIXELS_PER_THREAD, 0)
+            r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED)
+            assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=0), (family, force_clamp)
+            check_float_toplist(r["top"]["index"], want_w, 7)
 
 
 def test_multiple_breaks_per_band_fallback(bsh, torch, ctx):
@@ -203,29 +203,26 @@ def test_multiple_breaks_per_band_fallback(bsh, torch, ctx):
 @pytest.mark.parametrize("n_sft,n_f0,margin,f0,side", [(1, 1, 3, 50.0, 1), (33, 7, 12, 80.0, 3), (64, 90, 30, 120.0, 6),
                                                         (130, 97, 45, 150.0, 6), (70, 200, 60, 200.0, 3),
                                                         (2100, 64, 50, 180.0, 6), (8200, 33, 45, 150.0, 3)])
-def test_pixel_lane_kernel_ragged(bsh, torch, ctx, monkeypatch, n_sft, n_f0, margin, f0, side):
+def test_pixel_lane_kernel_ragged(bsh, torch, ctx, n_sft, n_f0, margin, f0, side):
     wl = synth.noise_workload(seed=1000 + n_sft + n_f0, n_sft=n_sft, n_f0=n_f0, margin=margin, f_band_start=f0,
                               n_pix_side=side, ap=(10.0, 40.0), P_days=(15.0, 31.0), n_t=3, topk=7)
     pk = oracle.peakgram(wl.rho)
     want_n, _ = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL, want_wcount=False)
-    monkeypatch.setenv("BSH_FORCE_PIX", "1")
+    ctx.set_option(bsh.BSH_OPT_KERNEL_FAMILY, bsh.BSH_FAMILY_PIXEL_LANE)
     for force_clamp in (False, True):
-        if force_clamp:
-            monkeypatch.setenv("BSH_FORCE_CLAMP", "1")
-        else:
-            monkeypatch.delenv("BSH_FORCE_CLAMP", raising=False)
+        ctx.set_option(bsh.BSH_OPT_FORCE_CLAMP, int(force_clamp))
         r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
         assert ctx.stats()["kernel_variant"] // 1000 == 2, "the pixel-lane kernel did not run"
         assert np.array_equal(r["counts"], want_n), force_clamp
         check_unweighted_toplist(r["top"], want_n, 7)
 
 
-def test_pixel_lane_kernel_multiple_breaks(bsh, torch, ctx, monkeypatch):
+def test_pixel_lane_kernel_multiple_breaks(bsh, torch, ctx):
     wl = synth.noise_workload(seed=78, n_sft=96, n_f0=90, margin=40, f_band_start=150.0, n_pix_side=2,
                               ap=(2500.0, 6000.0), P_days=(15.0,), n_t=4)
     pk = oracle.peakgram(wl.rho)
     want_n, _ = oracle.stage1(wl, pk, None, mode=oracle.CANONICAL)
-    monkeypatch.setenv("BSH_FORCE_PIX", "1")
+    ctx.set_option(bsh.BSH_OPT_KERNEL_FAMILY, bsh.BSH_FAMILY_PIXEL_LANE)
     r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
     assert ctx.stats()["kernel_variant"] // 1000 == 2
     assert np.array_equal(r["counts"], want_n)
@@ -427,20 +424,21 @@ def test_search_patch_host_end_to_end(bsh, torch, ctx):
     assert st["launches"] > 0 and st["n_templates"] == 1620
 
 
-def test_ties_round_to_even_on_the_gpu(bsh, torch, ctx, monkeypatch):
+def test_ties_round_to_even_on_the_gpu(bsh, torch, ctx):
     """R-1: exact half-integer bin coordinates (synth.tie_workload): every kernel family rounds them like the oracle."""
     wl = synth.tie_workload()
     pk = oracle.peakgram(wl.rho)
     want_n, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
-    for env in ({}, {"BSH_FORCE_PIX": "1"}, {"BSH_LEGACY": "1"}, {"BSH_FORCE_CLAMP": "1"}):
-        for key in ("BSH_FORCE_PIX", "BSH_LEGACY", "BSH_FORCE_CLAMP"):
-            monkeypatch.delenv(key, raising=False)
-        for key, val in env.items():
-            monkeypatch.setenv(key, val)
+    for env in ((bsh.BSH_FAMILY_AUTO, 0), (bsh.BSH_FAMILY_PIXEL_LANE, 0), (bsh.BSH_FAMILY_TEMPLATE_LANE, 0),
+                (bsh.BSH_FAMILY_WINDOW, 0), (bsh.BSH_FAMILY_AUTO, 1), (bsh.BSH_FAMILY_PIXEL_LANE, 1)):
+        ctx.set_option(bsh.BSH_OPT_KERNEL_FAMILY, env[0])
+        ctx.set_option(bsh.BSH_OPT_FORCE_CLAMP, env[1])
         r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
         assert np.array_equal(r["counts"], want_n), env
         r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED)
         assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=0), env
+    ctx.set_option(bsh.BSH_OPT_KERNEL_FAMILY, bsh.BSH_FAMILY_AUTO)
+    ctx.set_option(bsh.BSH_OPT_FORCE_CLAMP, 0)
     r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED | bsh.BSH_NAIVE)
     assert np.array_equal(r["counts"], want_n)
 
@@ -496,3 +494,55 @@ def test_fraction_nc_toplist_and_stage2(bsh, torch, ctx):
     pick = np.unique(np.concatenate([np.arange(200), rng.integers(0, k, 2000)]))
     want_p = oracle.stage2(wl2, recs["index"][pick], wl2.rho, wl2.w)
     assert np.allclose(recs["power"][pick], want_p, rtol=RTOL, atol=0)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# boundary extras: diagnostic options, measured peaks, state between launch and collect
+# ------------------------------------------------------------------------------------------------------------
+def test_set_option_validates(bsh, torch, ctx):
+    with pytest.raises(bsh.BshError):
+        ctx.set_option(99, 1)
+    with pytest.raises(bsh.BshError):
+        ctx.set_option(bsh.BSH_OPT_KERNEL_FAMILY, 7)
+    with pytest.raises(bsh.BshError):
+        ctx.set_option(bsh.BSH_OPT_PIXELS_PER_THREAD, 3)
+    ctx.set_option(bsh.BSH_OPT_KERNEL_FAMILY, bsh.BSH_FAMILY_AUTO)
+
+
+def test_measured_peaks_are_plausible(bsh, torch, ctx):
+    """bsh_measure_peaks: every rate must sit between half and 1.05x of the guide's unit counts for sm_100 (per SM and
+    clock: 128 FP32 lanes, 64 integer-ALU lanes, 128 B of shared memory, one warp instruction per scheduler)."""
+    pk = ctx.measure_peaks()
+    assert pk["n_sm"] == torch.cuda.get_device_properties(0).multi_processor_count
+    assert 1000 < pk["sm_clock_mhz"] < 2200
+    assert 0.5 < pk["issue_warp_inst_per_clk_smsp"] <= 1.02
+    assert 32 < pk["lop3_lanes_per_clk_sm"] <= 134
+    assert 64 < pk["fadd_lanes_per_clk_sm"] <= 134
+    assert 8 < pk["dadd_lanes_per_clk_sm"] <= 68 and 8 < pk["dmul_lanes_per_clk_sm"] <= 68
+    for k in ("lds32_bytes_per_clk_sm", "lds64_bytes_per_clk_sm", "lds128_bytes_per_clk_sm"):
+        assert 64 < pk[k] <= 134, (k, pk[k])
+
+
+def test_foreign_sft_sets_between_launch_and_collect(bsh, torch, ctx):
+    """The table cache holds two (SFT set, grid) entries; a launched, uncollected stage 1 must keep its entry while
+    stage 2 runs on two OTHER SFT sets in between (the LRU slot could be the pending call's)."""
+    wl = synth.noise_workload(seed=701, n_sft=300, n_f0=90, margin=45, f_band_start=150.0, n_pix_side=6,
+                              ap=(10.0, 25.0, 40.0), P_days=(15.0, 31.0), n_t=4, topk=50)
+    pk = oracle.peakgram(wl.rho)
+    want_n, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
+    d_rho, d_w = dev(torch, wl.rho), dev(torch, wl.w)
+    d_peak = ctx.build_peakgram(d_rho)
+    # a first toplist to feed the foreign stage-2 calls
+    d_top0, n0 = ctx.stage1_hough(d_peak, wl, topk=50, d_w=d_w)
+    others = [synth.overlapped_stage2_set(wl, seed=s) for s in (702, 703)]
+    counts = torch.full((wl.n_templates,), -7, dtype=torch.int32, device="cuda")
+    ctx.stage1_launch(d_peak, wl, mode=bsh.BSH_UNWEIGHTED, topk=50, d_w=d_w, counts_full=counts)
+    for o in others:                                           # two different SFT sets: both cache slots are wanted
+        d_r, d_ww = dev(torch, o.rho), dev(torch, o.w)
+        ctx.stage2_power(d_r, o, d_top0, n0, d_w=d_ww, sort_by_power=False)
+    d_top, n_top = ctx.stage1_collect()
+    torch.cuda.synchronize()
+    assert np.array_equal(counts.cpu().numpy(), want_n)
+    top = ctx.records(d_top, n_top)
+    check_unweighted_toplist(top, want_n, 50)
+    assert np.allclose(top["wcount"], want_w[top["index"].astype(np.int64)], rtol=RTOL, atol=0)
