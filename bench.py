@@ -137,10 +137,16 @@ def oracle_subgrid(wl, seconds: float, n_threads: int = 0):
     mode (Eq. 15 with one libm cos per accumulation) finishes in ~`seconds` on n_threads (0 = all cores)."""
     import oracle
     pk = oracle.peakgram(wl.rho)
-    probe = wl.subgrid(ia=[0], ip=[0], it=[0, 1], pix=[0, 1])
-    t0 = time.perf_counter()
-    oracle.stage1(probe, pk, wl.w, mode=oracle.DIRECT, n_threads=n_threads)
-    rate = probe.n_accumulations / max(time.perf_counter() - t0, 1e-6)
+    n_it, rate = 2, 0.0
+    while True:                                             # probe until the run is long enough to time (>= 0.3 s)
+        probe = wl.subgrid(ia=[0], ip=[0], it=list(range(min(n_it, len(wl.tasc_frac)))), pix=list(range(min(8, wl.n_pix))))
+        t0 = time.perf_counter()
+        oracle.stage1(probe, pk, wl.w, mode=oracle.DIRECT, n_threads=n_threads)
+        dt = time.perf_counter() - t0
+        rate = probe.n_accumulations / max(dt, 1e-6)
+        if dt >= 0.3 or n_it >= len(wl.tasc_frac):
+            break
+        n_it *= 4
     n_b = int(max(2, min(wl.n_binary * wl.n_pix, rate * seconds / (wl.n_f0 * wl.n_sft))))
     n_it = min(len(wl.tasc_frac), max(1, n_b // 8))
     n_pix = min(wl.n_pix, max(1, n_b // n_it))

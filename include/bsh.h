@@ -115,8 +115,8 @@ typedef struct {
 typedef struct {
     int32_t n_sm;                          /* multiprocessors                                                     */
     double  sm_clock_mhz;                  /* SM clock during the measurement (clock64 against globaltimer)       */
-    double  issue_warp_inst_per_clk_smsp;  /* alternating LOP3 / FADD stream: warp instructions per clock per     */
-                                           /*   scheduler (SM sub-partition); lanes/clk/SM = 128 x this           */
+    double  issue_warp_inst_per_clk_smsp;  /* 1 LOP3 : 3 FADD stream: warp instructions per clock per scheduler   */
+                                           /*   (SM sub-partition); lanes/clk/SM = 128 x this                     */
     double  lop3_lanes_per_clk_sm;         /* integer-ALU pipe (bit-sliced counters)                              */
     double  fadd_lanes_per_clk_sm;         /* predicated FP32 add (weighted number count, L223)                   */
     double  dadd_lanes_per_clk_sm;         /* FP64 add, no FMA (canonical track, R-5)                             */

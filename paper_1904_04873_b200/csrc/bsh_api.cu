@@ -617,17 +617,17 @@ int bsh_measure_peaks(bsh_ctx *ctx, bsh_peaks *h_out)
     bsh_peaks pk = {};
     pk.n_sm = n_sm;
     double mhz[4] = {0, 0, 0, 0}, v = 0;
-    TRY(run_peak<kOpLop3>(ctx, n_sm, 4000, host, &pk.lop3_lanes_per_clk_sm, &mhz[0]));
-    TRY(run_peak<kOpFadd>(ctx, n_sm, 4000, host, &pk.fadd_lanes_per_clk_sm, &mhz[1]));
-    TRY(run_peak<kOpDadd>(ctx, n_sm, 2000, host, &pk.dadd_lanes_per_clk_sm, &mhz[2]));
-    TRY(run_peak<kOpDmul>(ctx, n_sm, 2000, host, &pk.dmul_lanes_per_clk_sm, nullptr));
-    TRY(run_peak<kOpMixed>(ctx, n_sm, 4000, host, &v, &mhz[3]));
+    TRY(run_peak<kOpLop3>(ctx, n_sm, 1000, host, &pk.lop3_lanes_per_clk_sm, &mhz[0]));
+    TRY(run_peak<kOpFadd>(ctx, n_sm, 1000, host, &pk.fadd_lanes_per_clk_sm, &mhz[1]));
+    TRY(run_peak<kOpDadd>(ctx, n_sm, 500, host, &pk.dadd_lanes_per_clk_sm, &mhz[2]));
+    TRY(run_peak<kOpDmul>(ctx, n_sm, 500, host, &pk.dmul_lanes_per_clk_sm, nullptr));
+    TRY(run_peak<kOpMixed>(ctx, n_sm, 1000, host, &v, &mhz[3]));
     pk.issue_warp_inst_per_clk_smsp = v / 32.0 / 4.0;
-    TRY(run_peak<kOpLds32>(ctx, n_sm, 2000, host, &v, nullptr));
+    TRY(run_peak<kOpLds32>(ctx, n_sm, 500, host, &v, nullptr));
     pk.lds32_bytes_per_clk_sm = 4.0 * v;
-    TRY(run_peak<kOpLds64>(ctx, n_sm, 2000, host, &v, nullptr));
+    TRY(run_peak<kOpLds64>(ctx, n_sm, 500, host, &v, nullptr));
     pk.lds64_bytes_per_clk_sm = 8.0 * v;
-    TRY(run_peak<kOpLds128>(ctx, n_sm, 1000, host, &v, nullptr));
+    TRY(run_peak<kOpLds128>(ctx, n_sm, 250, host, &v, nullptr));
     pk.lds128_bytes_per_clk_sm = 16.0 * v;
     std::sort(mhz, mhz + 4);
     pk.sm_clock_mhz = 0.5 * (mhz[1] + mhz[2]);

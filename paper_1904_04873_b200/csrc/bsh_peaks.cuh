@@ -13,7 +13,7 @@
 namespace bsh {
 
 constexpr int kPeakThreads = 1024;    // one block of 32 warps per SM: 8 warps per scheduler
-constexpr int kPeakUnroll = 64;       // operations per thread per loop iteration
+constexpr int kPeakUnroll = 256;      // operations per thread per loop iteration (loop overhead: ~1 %)
 
 enum PeakOp { kOpLop3 = 0, kOpFadd, kOpDadd, kOpDmul, kOpMixed, kOpLds32, kOpLds64, kOpLds128, kOpCount };
 
@@ -22,7 +22,7 @@ struct PeakSample {
     unsigned long long ns;            // globaltimer delta of the block
 };
 
-#define BSH_REP8(X) X X X X X X X X
+#define BSH_REP8(X) X X X X X X X X X X X X X X X X X X X X X X X X X X X X X X X X   /* 32 x 8 operations */
 
 template <int OP>
 __global__ void __launch_bounds__(kPeakThreads, 1) peak_kernel(int iters, uint32_t seed, uint32_t *sink, PeakSample *samples)
@@ -72,29 +72,29 @@ __global__ void __launch_bounds__(kPeakThreads, 1) peak_kernel(int iters, uint32
                                   : "+d"(d0), "+d"(d1), "+d"(d2), "+d"(d3), "+d"(d4), "+d"(d5), "+d"(d6), "+d"(d7)
                                   : "d"(dm));)
         } else if (OP == kOpMixed) {
-            // issue-rate probe: integer-ALU and FP32 instructions alternate, so neither pipe alone is the limit
-            BSH_REP8(asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;\n\tadd.f32 %4, %4, %8;\n\t"
-                                  "lop3.b32 %1, %1, %2, %3, 0x96;\n\tadd.f32 %5, %5, %8;\n\t"
-                                  "lop3.b32 %2, %2, %3, %0, 0x96;\n\tadd.f32 %6, %6, %8;\n\t"
-                                  "lop3.b32 %3, %3, %0, %1, 0x96;\n\tadd.f32 %7, %7, %8;"
-                                  : "+r"(r0), "+r"(r1), "+r"(r2), "+r"(r3), "+f"(f4), "+f"(f5), "+f"(f6), "+f"(f7)
+            // issue-rate probe: one integer-ALU instruction per three FP32 adds, so that neither pipe alone is the limit
+            // (the ALU pipe takes a warp instruction every other clock, the FP32 pipe one per clock)
+            BSH_REP8(asm volatile("lop3.b32 %0, %0, %1, %0, 0x96;\n\tadd.f32 %2, %2, %8;\n\tadd.f32 %3, %3, %8;\n\t"
+                                  "add.f32 %4, %4, %8;\n\tlop3.b32 %1, %1, %0, %1, 0x96;\n\tadd.f32 %5, %5, %8;\n\t"
+                                  "add.f32 %6, %6, %8;\n\tadd.f32 %7, %7, %8;"
+                                  : "+r"(r0), "+r"(r1), "+f"(f2), "+f"(f3), "+f"(f4), "+f"(f5), "+f"(f6), "+f"(f7)
                                   : "f"(fw));)
         } else if (OP == kOpLds32) {
-            BSH_REP8(asm volatile("ld.shared.u32 %0, [%4];\n\tld.shared.u32 %1, [%4+4096];\n\tld.shared.u32 %2, [%4+8192];\n\t"
-                                  "ld.shared.u32 %3, [%4+12288];\n\tld.shared.u32 %0, [%4];\n\tld.shared.u32 %1, [%4+4096];\n\t"
-                                  "ld.shared.u32 %2, [%4+8192];\n\tld.shared.u32 %3, [%4+12288];"
+            BSH_REP8(asm volatile("ld.volatile.shared.u32 %0, [%4];\n\tld.volatile.shared.u32 %1, [%4+4096];\n\tld.volatile.shared.u32 %2, [%4+8192];\n\t"
+                                  "ld.volatile.shared.u32 %3, [%4+12288];\n\tld.volatile.shared.u32 %0, [%4];\n\tld.volatile.shared.u32 %1, [%4+4096];\n\t"
+                                  "ld.volatile.shared.u32 %2, [%4+8192];\n\tld.volatile.shared.u32 %3, [%4+12288];"
                                   : "=r"(l0), "=r"(l1), "=r"(l2), "=r"(l3) : "r"(a4));)
         } else if (OP == kOpLds64) {
-            BSH_REP8(asm volatile("ld.shared.v2.u32 {%0,%1}, [%4];\n\tld.shared.v2.u32 {%2,%3}, [%4+8192];\n\t"
-                                  "ld.shared.v2.u32 {%0,%1}, [%4];\n\tld.shared.v2.u32 {%2,%3}, [%4+8192];\n\t"
-                                  "ld.shared.v2.u32 {%0,%1}, [%4];\n\tld.shared.v2.u32 {%2,%3}, [%4+8192];\n\t"
-                                  "ld.shared.v2.u32 {%0,%1}, [%4];\n\tld.shared.v2.u32 {%2,%3}, [%4+8192];"
+            BSH_REP8(asm volatile("ld.volatile.shared.v2.u32 {%0,%1}, [%4];\n\tld.volatile.shared.v2.u32 {%2,%3}, [%4+8192];\n\t"
+                                  "ld.volatile.shared.v2.u32 {%0,%1}, [%4];\n\tld.volatile.shared.v2.u32 {%2,%3}, [%4+8192];\n\t"
+                                  "ld.volatile.shared.v2.u32 {%0,%1}, [%4];\n\tld.volatile.shared.v2.u32 {%2,%3}, [%4+8192];\n\t"
+                                  "ld.volatile.shared.v2.u32 {%0,%1}, [%4];\n\tld.volatile.shared.v2.u32 {%2,%3}, [%4+8192];"
                                   : "=r"(l0), "=r"(l1), "=r"(l2), "=r"(l3) : "r"(a8));)
         } else {
-            BSH_REP8(asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\t"
-                                  "ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\t"
-                                  "ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\t"
-                                  "ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.shared.v4.u32 {%0,%1,%2,%3}, [%4];"
+            BSH_REP8(asm volatile("ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\t"
+                                  "ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\t"
+                                  "ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\t"
+                                  "ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];"
                                   : "=r"(l0), "=r"(l1), "=r"(l2), "=r"(l3) : "r"(a16));)
         }
     }
