@@ -17,6 +17,7 @@
 #include "bsh_kernels.cuh"
 #include "bsh_pos.cuh"
 #include "bsh_pix.cuh"
+#include "bsh_wpix.cuh"
 #include "bsh_peaks.cuh"
 
 using namespace bsh;
@@ -63,6 +64,9 @@ struct Pending {                      // state between bsh_stage1_launch and bsh
     // pixel-lane kernel (bsh_pix.cuh)
     bool use_pix = false;
     int n_pg = 0, pix_stages = 0, pix_smem = 0;
+    // weighted pixel-lane kernel (bsh_wpix.cuh)
+    bool use_wpix = false;
+    int wpix_nbytes = 0, wpix_stages = 0, wpix_smem = 0;
 };
 
 }  // namespace
@@ -73,7 +77,7 @@ struct bsh_ctx {
     std::string err;
     TableCache cache[2];
     uint64_t stamp = 0;
-    DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2, ptab, dpos, dpix, psplit;
+    DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2, ptab, dpos, dpix, psplit, tab7;
     DevBuf h_rho, h_w, h_peak, h_top;                  // device staging of bsh_search_patch_host
     unsigned int *pinned_count = nullptr;
     cudaEvent_t ev[10] = {};
@@ -345,6 +349,19 @@ int dispatch_weighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p, i
     return fail(ctx, BSH_EINVAL, "no weighted position kernel for NW=%d", pd.NW);
 }
 
+#define W_PIX_CASE(NBYTES_, CL_)                                                                      \
+    if (pd.wpix_nbytes == NBYTES_ && pd.clamp == CL_)                                                 \
+        return launch_stage1(ctx, stage1_weighted_pix_kernel<NBYTES_, CL_>, p, 32 * kWpixWarps, grid, pd.wpix_smem);
+
+int dispatch_weighted_pix(bsh_ctx *ctx, const Pending &pd, const WpixParams &p, int grid)
+{
+    W_PIX_CASE(13, false)
+#ifndef BSH_MINIMAL
+    W_PIX_CASE(13, true) W_PIX_CASE(8, false) W_PIX_CASE(8, true)
+#endif
+    return fail(ctx, BSH_EINVAL, "no weighted pixel-lane kernel for %d bytes clamp=%d", pd.wpix_nbytes, (int)pd.clamp);
+}
+
 // one accumulation pass over all f0 tiles with the current threshold shift
 int run_pass(bsh_ctx *ctx)
 {
@@ -371,6 +388,35 @@ int run_pass(bsh_ctx *ctx)
         CK(cudaGetLastError());
         ctx->st.grid_blocks = (int)blocks;
         ctx->st.threads_per_block = 256;
+    } else if (pd.use_wpix && weighted) {
+        const int tile_bins = pd.tile_bins;
+        for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
+            WpixParams p;
+            p.tab7 = (const unsigned char *)ctx->tab7.p;
+            p.cs = (const double2 *)c.d_cs.p;
+            p.dpix = (const double *)ctx->dpix.p;
+            p.w_pad = (const float *)ctx->w_pad.p;
+            p.A = (const double *)c.d_A.p;
+            p.casa = (const double2 *)c.d_casa.p;
+            p.n_pad = pd.n_pad; p.n_pos = pd.n_pos; p.n_chunks = pd.n_pad / kStageSfts; p.n_stages = pd.wpix_stages;
+            p.n_pix = pd.n_pix; p.n_ap = pd.n_ap; p.n_P = pd.n_P; p.n_tasc = pd.n_tasc; p.n_f0 = pd.n_f0;
+            p.j0 = j0; p.n_fj = std::min(tile_bins, pd.n_f0 - j0);
+            p.n_pg = pd.n_pg; p.n_aq = pd.n_ap * pd.n_tasc; p.n_aq_tiles = (p.n_aq + kWpixWarps - 1) / kWpixWarps;
+            p.u0 = (double)(pd.k_band0 + j0);
+            p.off = (int)(pd.k_band0 - pd.k_slab0) + j0 + pd.pos_off;
+            p.s_max = pd.pos_s_max;
+            p.s_zero = pd.pos_s_zero;
+            p.thr = (const Threshold *)ctx->thr.p;
+            p.cand = (RawCand *)ctx->cand.p;
+            p.cand_count = (unsigned int *)ctx->cand_count.p;
+            p.cand_cap = pd.cand_cap;
+            p.counts_full = pd.d_counts_full;
+            const int64_t grid = (int64_t)pd.n_pg * pd.n_P * p.n_aq_tiles;
+            if (grid > 0x7FFFFFFFll) return fail(ctx, BSH_EINVAL, "grid too large");
+            ctx->st.grid_blocks = (int)grid;
+            ctx->st.threads_per_block = 32 * kWpixWarps;
+            TRY(dispatch_weighted_pix(ctx, pd, p, (int)grid));
+        }
     } else if (pd.use_pix && !weighted) {
         const int tile_bins = pd.tile_bins;
         for (int j0 = 0; j0 < pd.n_f0; j0 += tile_bins) {
@@ -552,7 +598,7 @@ int bsh_destroy(bsh_ctx *ctx)
     const DeviceGuard device_guard(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf *bufs[] = {&ctx->wtab, &ctx->w_pad, &ctx->stats, &ctx->thr, &ctx->dtab, &ctx->nvec, &ctx->cand, &ctx->cand_count,
-                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->psplit, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top, &ctx->peak_samples};
+                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->psplit, &ctx->tab7, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top, &ctx->peak_samples};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto &c : ctx->cache) {
@@ -696,6 +742,28 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         pd.NW = 2;
         pd.tile_bins = (grid->n_f0 + 1) / 2;
     }
+    // weighted pixel-lane kernel (bsh_wpix.cuh): one pass over tiles of <= 91 bins (13 bytes of 7 bins; 8 bytes for <= 56)
+    pd.n_pg = (grid->n_pix + 31) / 32;
+    const bool lanes_ok = 10 * grid->n_pix >= 6 * 32 * pd.n_pg;
+    const int fam = ctx->opt_family;
+    bool try_wpix = weighted && !(mode & BSH_NAIVE) && ((fam == BSH_FAMILY_AUTO && lanes_ok) || fam == BSH_FAMILY_PIXEL_LANE);
+    if (try_wpix) {
+        const int n_tiles = (grid->n_f0 + 90) / 91;
+        const int tile = (grid->n_f0 + n_tiles - 1) / n_tiles;
+        const int nbytes = tile <= 56 ? 8 : 13, nw = nbytes == 8 ? 2 : 3;
+        const TableGeometry tgw = table_geometry(sfts->n_sft, sfts->h_v_over_c, grid->n_P, grid->h_P, grid->n_ap, grid->h_ap,
+                                                 grid->k_band0, sfts->k_slab0, grid->n_f0, sfts->n_bins, nw,
+                                                 ctx->opt_force_clamp != 0);
+        const PosGeometry pgw = pos_geometry(tgw, sfts->n_bins, grid->n_f0, nw, tile);
+        const WpixStage ws(pgw.n_pos, wpix_entry_bytes(nbytes));
+        const int stages = std::min(kMaxStages, (220 * 1024 - kWpixHeader) / ws.stride);     // one block per SM
+        if (stages >= 2) {
+            pd.use_wpix = true;
+            pd.tile_bins = tile; pd.wpix_nbytes = nbytes; pd.NW = nw;
+            pd.wpix_stages = std::max(1, std::min(stages, pd.n_pad / kStageSfts));
+            pd.wpix_smem = ws.total(pd.wpix_stages);
+        }
+    }
     if (!weighted && (ctx->opt_pixels_per_thread == 1 || ctx->opt_pixels_per_thread == 2)) pd.R = ctx->opt_pixels_per_thread;
     pd.HP = sfts->n_sft < (1 << 11) ? 6 : (sfts->n_sft < (1 << 13) ? 8 : 11);
     if (sfts->n_sft >= (1 << 16)) return fail(ctx, BSH_EINVAL, "n_sft >= 65536 not supported");
@@ -718,7 +786,6 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         const int budgets[3] = {112 * 1024, 112 * 1024, 224 * 1024};                          // 2 / 2 / 1 blocks per SM
         pd.n_stages = 0;
         for (int b = 0; b < 3 && pd.n_stages < 2; ++b) pd.n_stages = std::min(kMaxStages, (budgets[b] - kPosHeader) / stride);
-        const int fam = ctx->opt_family;
         pd.use_pos = pd.n_stages >= 2 && fam != BSH_FAMILY_WINDOW && !(mode & BSH_NAIVE);
         pd.n_stages = std::min(pd.n_stages, pd.n_pad / kStageSfts);
         pd.pos_groups = weighted ? grid->n_pix : (grid->n_pix + 1) / 2;
@@ -726,12 +793,10 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         pd.pos_smem = kPosHeader + pd.n_stages * stride;
         // pixel-lane kernel (unweighted): pixels on the lanes pay off when most of the 32 lanes of a group are used
         const PixStage ps(pg.n_pos);
-        pd.n_pg = (grid->n_pix + 31) / 32;
         pd.pix_stages = 0;
         const int hi_bytes = pix_hi_bytes(pd.NW, pd.HP);                                    // shared-memory high planes
         for (int b = 1; b < 3 && pd.pix_stages < 2; ++b)
             pd.pix_stages = std::min(4, (budgets[b] - kPixHeader - hi_bytes) / ps.stride);      // (2..6 stages measure alike)
-        const bool lanes_ok = 10 * grid->n_pix >= 6 * 32 * pd.n_pg;
         pd.use_pix = !weighted && pd.pix_stages >= 2 && (lanes_ok || fam == BSH_FAMILY_PIXEL_LANE) &&
                      (fam == BSH_FAMILY_AUTO || fam == BSH_FAMILY_PIXEL_LANE) && !(mode & BSH_NAIVE);
         pd.pix_stages = std::max(1, std::min(pd.pix_stages, pd.n_pad / kStageSfts));
@@ -767,7 +832,27 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     count_launch(ctx);
     CK(cudaGetLastError());
     TRY(build_dtable(ctx, grid, c, pd.R, ctx->nvec, ctx->dtab));
-    if (pd.use_pix) {
+    if (pd.use_wpix) {
+        const int eb = wpix_entry_bytes(pd.wpix_nbytes);
+        const int64_t n_ent = (int64_t)pd.n_pad * pd.n_pos;
+        TRY(ensure(ctx, ctx->tab7, (size_t)(pd.n_pad / kStageSfts) * (size_t)wpix_stage_tab_bytes(pd.n_pos, eb)));
+        TRY(ensure(ctx, ctx->dpix, sizeof(double) * (size_t)pd.n_pg * pd.n_pad * 32));
+        if (eb == 8)
+            build_position7_table_kernel<8><<<(unsigned)((n_ent + 255) / 256), 256, 0, ctx->stream>>>(
+                d_peak, words_per_row, sfts->n_sft, pd.n_pad, sfts->n_bins, pd.n_pos, pd.pos_off, pd.pos_s_zero,
+                (unsigned char *)ctx->tab7.p);
+        else
+            build_position7_table_kernel<16><<<(unsigned)((n_ent + 255) / 256), 256, 0, ctx->stream>>>(
+                d_peak, words_per_row, sfts->n_sft, pd.n_pad, sfts->n_bins, pd.n_pos, pd.pos_off, pd.pos_s_zero,
+                (unsigned char *)ctx->tab7.p);
+        count_launch(ctx);
+        const int64_t n_d = (int64_t)pd.n_pg * pd.n_pad * 32;
+        dtable_pix_kernel<<<(unsigned)((n_d + 255) / 256), 256, 0, ctx->stream>>>(
+            (const double *)c.d_v.p, (const double *)ctx->nvec.p, c.n_sft, pd.n_pad, grid->n_pix, pd.n_pg,
+            (double *)ctx->dpix.p);
+        count_launch(ctx);
+        CK(cudaGetLastError());
+    } else if (pd.use_pix) {
         TRY(ensure(ctx, ctx->ptab, (size_t)pd.n_pad * pd.n_pos * 16));
         TRY(ensure(ctx, ctx->dpix, sizeof(double) * (size_t)pd.n_pg * pd.n_pad * 32));
         const int64_t n_ent = (int64_t)pd.n_pad * pd.n_pos;
@@ -814,7 +899,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
 
     ctx->st.n_templates = (int64_t)pd.n_templates;
     ctx->st.n_accumulations = (int64_t)pd.n_templates * sfts->n_sft;
-    ctx->st.kernel_variant = (pd.use_pix ? 2000 : pd.use_pos ? 1000 : 0) + pd.NW * 100 + pd.R * 10 + (pd.clamp ? 1 : 0);
+    ctx->st.kernel_variant = (pd.use_wpix ? 3000 : pd.use_pix ? 2000 : pd.use_pos ? 1000 : 0) + pd.NW * 100 + pd.R * 10 + (pd.clamp ? 1 : 0);
     return BSH_OK;
 }
 

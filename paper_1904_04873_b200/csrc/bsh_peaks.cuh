@@ -27,8 +27,8 @@ struct PeakSample {
 template <int OP>
 __global__ void __launch_bounds__(kPeakThreads, 1) peak_kernel(int iters, uint32_t seed, uint32_t *sink, PeakSample *samples)
 {
-    __shared__ __align__(16) uint32_t sm[kPeakThreads * 4];
-    for (int i = threadIdx.x; i < kPeakThreads * 4; i += blockDim.x) sm[i] = i * 2654435761u + seed;
+    __shared__ __align__(16) uint32_t sm[kPeakThreads * 8];
+    for (int i = threadIdx.x; i < kPeakThreads * 8; i += blockDim.x) sm[i] = i * 2654435761u + seed;
     __syncthreads();
     uint32_t r0 = threadIdx.x + seed, r1 = r0 * 3u, r2 = r0 * 5u, r3 = r0 * 7u, r4 = r0 * 11u, r5 = r0 * 13u, r6 = r0 * 17u, r7 = r0 * 19u;
     float f0 = 1.f + r0 * 1e-9f, f1 = f0 + 1.f, f2 = f0 + 2.f, f3 = f0 + 3.f, f4 = f0 + 4.f, f5 = f0 + 5.f, f6 = f0 + 6.f, f7 = f0 + 7.f;
@@ -80,22 +80,41 @@ __global__ void __launch_bounds__(kPeakThreads, 1) peak_kernel(int iters, uint32
                                   : "+r"(r0), "+r"(r1), "+f"(f2), "+f"(f3), "+f"(f4), "+f"(f5), "+f"(f6), "+f"(f7)
                                   : "f"(fw));)
         } else if (OP == kOpLds32) {
-            BSH_REP8(asm volatile("ld.volatile.shared.u32 %0, [%4];\n\tld.volatile.shared.u32 %1, [%4+4096];\n\tld.volatile.shared.u32 %2, [%4+8192];\n\t"
-                                  "ld.volatile.shared.u32 %3, [%4+12288];\n\tld.volatile.shared.u32 %0, [%4];\n\tld.volatile.shared.u32 %1, [%4+4096];\n\t"
-                                  "ld.volatile.shared.u32 %2, [%4+8192];\n\tld.volatile.shared.u32 %3, [%4+12288];"
-                                  : "=r"(l0), "=r"(l1), "=r"(l2), "=r"(l3) : "r"(a4));)
+            // every loaded word is consumed (3-input XOR into four chains), so no load can be dropped or merged
+            BSH_REP8(asm volatile("{\n\t.reg .b32 t<8>;\n\t"
+                                  "ld.volatile.shared.u32 t0, [%4];\n\tld.volatile.shared.u32 t1, [%4+4096];\n\t"
+                                  "ld.volatile.shared.u32 t2, [%4+8192];\n\tld.volatile.shared.u32 t3, [%4+12288];\n\t"
+                                  "ld.volatile.shared.u32 t4, [%4+16384];\n\tld.volatile.shared.u32 t5, [%4+20480];\n\t"
+                                  "ld.volatile.shared.u32 t6, [%4+24576];\n\tld.volatile.shared.u32 t7, [%4+28672];\n\t"
+                                  "lop3.b32 %0, %0, t0, t1, 0x96;\n\tlop3.b32 %1, %1, t2, t3, 0x96;\n\t"
+                                  "lop3.b32 %2, %2, t4, t5, 0x96;\n\tlop3.b32 %3, %3, t6, t7, 0x96;\n\t}"
+                                  : "+r"(l0), "+r"(l1), "+r"(l2), "+r"(l3) : "r"(a4));)
         } else if (OP == kOpLds64) {
-            BSH_REP8(asm volatile("ld.volatile.shared.v2.u32 {%0,%1}, [%4];\n\tld.volatile.shared.v2.u32 {%2,%3}, [%4+8192];\n\t"
-                                  "ld.volatile.shared.v2.u32 {%0,%1}, [%4];\n\tld.volatile.shared.v2.u32 {%2,%3}, [%4+8192];\n\t"
-                                  "ld.volatile.shared.v2.u32 {%0,%1}, [%4];\n\tld.volatile.shared.v2.u32 {%2,%3}, [%4+8192];\n\t"
-                                  "ld.volatile.shared.v2.u32 {%0,%1}, [%4];\n\tld.volatile.shared.v2.u32 {%2,%3}, [%4+8192];"
-                                  : "=r"(l0), "=r"(l1), "=r"(l2), "=r"(l3) : "r"(a8));)
+            BSH_REP8(asm volatile("{\n\t.reg .b32 t<16>;\n\t"
+                                  "ld.volatile.shared.v2.u32 {t0,t1}, [%4];\n\tld.volatile.shared.v2.u32 {t2,t3}, [%4+8192];\n\t"
+                                  "ld.volatile.shared.v2.u32 {t4,t5}, [%4+16384];\n\tld.volatile.shared.v2.u32 {t6,t7}, [%4+24576];\n\t"
+                                  "ld.volatile.shared.v2.u32 {t8,t9}, [%4];\n\tld.volatile.shared.v2.u32 {t10,t11}, [%4+8192];\n\t"
+                                  "ld.volatile.shared.v2.u32 {t12,t13}, [%4+16384];\n\tld.volatile.shared.v2.u32 {t14,t15}, [%4+24576];\n\t"
+                                  "lop3.b32 %0, %0, t0, t1, 0x96;\n\tlop3.b32 %1, %1, t2, t3, 0x96;\n\t"
+                                  "lop3.b32 %2, %2, t4, t5, 0x96;\n\tlop3.b32 %3, %3, t6, t7, 0x96;\n\t"
+                                  "lop3.b32 %0, %0, t8, t9, 0x96;\n\tlop3.b32 %1, %1, t10, t11, 0x96;\n\t"
+                                  "lop3.b32 %2, %2, t12, t13, 0x96;\n\tlop3.b32 %3, %3, t14, t15, 0x96;\n\t}"
+                                  : "+r"(l0), "+r"(l1), "+r"(l2), "+r"(l3) : "r"(a8));)
         } else {
-            BSH_REP8(asm volatile("ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\t"
-                                  "ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\t"
-                                  "ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\t"
-                                  "ld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];\n\tld.volatile.shared.v4.u32 {%0,%1,%2,%3}, [%4];"
-                                  : "=r"(l0), "=r"(l1), "=r"(l2), "=r"(l3) : "r"(a16));)
+            BSH_REP8(asm volatile("{\n\t.reg .b32 t<32>;\n\t"
+                                  "ld.volatile.shared.v4.u32 {t0,t1,t2,t3}, [%4];\n\tld.volatile.shared.v4.u32 {t4,t5,t6,t7}, [%4+16384];\n\t"
+                                  "ld.volatile.shared.v4.u32 {t8,t9,t10,t11}, [%4];\n\tld.volatile.shared.v4.u32 {t12,t13,t14,t15}, [%4+16384];\n\t"
+                                  "ld.volatile.shared.v4.u32 {t16,t17,t18,t19}, [%4];\n\tld.volatile.shared.v4.u32 {t20,t21,t22,t23}, [%4+16384];\n\t"
+                                  "ld.volatile.shared.v4.u32 {t24,t25,t26,t27}, [%4];\n\tld.volatile.shared.v4.u32 {t28,t29,t30,t31}, [%4+16384];\n\t"
+                                  "lop3.b32 %0, %0, t0, t1, 0x96;\n\tlop3.b32 %1, %1, t2, t3, 0x96;\n\t"
+                                  "lop3.b32 %2, %2, t4, t5, 0x96;\n\tlop3.b32 %3, %3, t6, t7, 0x96;\n\t"
+                                  "lop3.b32 %0, %0, t8, t9, 0x96;\n\tlop3.b32 %1, %1, t10, t11, 0x96;\n\t"
+                                  "lop3.b32 %2, %2, t12, t13, 0x96;\n\tlop3.b32 %3, %3, t14, t15, 0x96;\n\t"
+                                  "lop3.b32 %0, %0, t16, t17, 0x96;\n\tlop3.b32 %1, %1, t18, t19, 0x96;\n\t"
+                                  "lop3.b32 %2, %2, t20, t21, 0x96;\n\tlop3.b32 %3, %3, t22, t23, 0x96;\n\t"
+                                  "lop3.b32 %0, %0, t24, t25, 0x96;\n\tlop3.b32 %1, %1, t26, t27, 0x96;\n\t"
+                                  "lop3.b32 %2, %2, t28, t29, 0x96;\n\tlop3.b32 %3, %3, t30, t31, 0x96;\n\t}"
+                                  : "+r"(l0), "+r"(l1), "+r"(l2), "+r"(l3) : "r"(a16));)
         }
     }
     // keep every chain alive

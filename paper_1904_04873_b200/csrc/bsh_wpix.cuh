@@ -41,6 +41,8 @@ __host__ __device__ constexpr int wpix_entry_bytes(int nbytes) { return nbytes <
 // triple, the SFT part an instruction immediate -- and (ii) neighbouring positions start 4 (2) banks apart: the 8 lanes
 // a 16-byte (8-byte: 16 lanes) shared-memory wavefront serves read neighbouring positions without bank conflicts.
 __host__ __device__ constexpr int wpix_record_bytes(int eb) { return (kStageSfts + 1) * eb; }
+// bytes of one stage of the table (n_pos records), rounded up to the 16 bytes a bulk copy moves
+__host__ __device__ constexpr int64_t wpix_stage_tab_bytes(int n_pos, int eb) { return ((int64_t)n_pos * wpix_record_bytes(eb) + 15) & ~(int64_t)15; }
 
 // 7-bins-per-byte position table: entry p of SFT i = the window STARTING at table position p (slab column p - off_table),
 // bin j in bit (j % 7) of byte (j / 7); bits outside [0, K), the padding SFTs and position s_zero are zero.
@@ -74,7 +76,8 @@ __global__ void __launch_bounds__(256) build_position7_table_kernel(const uint32
         if (s > 25 && w + 1 < 4) bits |= v[w + 1] << (32 - s);
         out[q >> 2] |= (bits & 0x7Fu) << (8 * (q & 3));
     }
-    unsigned char *dst = tab + ((int64_t)(i / kStageSfts) * n_pos + p) * wpix_record_bytes(EB) + (i % kStageSfts) * EB;
+    unsigned char *dst = tab + (int64_t)(i / kStageSfts) * wpix_stage_tab_bytes(n_pos, EB) + (int64_t)p * wpix_record_bytes(EB) +
+                         (i % kStageSfts) * EB;
     if (EB == 8) *reinterpret_cast<uint2 *>(dst) = make_uint2(out[0], out[1]);
     else *reinterpret_cast<uint4 *>(dst) = make_uint4(out[0], out[1], out[2], out[3]);
     if (i % kStageSfts == 0) {                           // the record's padding entry
@@ -87,7 +90,7 @@ __global__ void __launch_bounds__(256) build_position7_table_kernel(const uint32
 template <int EB>
 __device__ __forceinline__ const unsigned char *entry7(const unsigned char *tab, int n_pos, int i, int s)
 {
-    return tab + ((int64_t)(i / kStageSfts) * n_pos + s) * wpix_record_bytes(EB) + (i % kStageSfts) * EB;
+    return tab + (int64_t)(i / kStageSfts) * wpix_stage_tab_bytes(n_pos, EB) + (int64_t)s * wpix_record_bytes(EB) + (i % kStageSfts) * EB;
 }
 
 struct WpixParams {
@@ -114,7 +117,7 @@ struct WpixStage {
     int tab_bytes, cs_bytes, d_bytes, w_bytes, stride;
     __device__ __host__ WpixStage(int n_pos, int eb)
     {
-        tab_bytes = n_pos * wpix_record_bytes(eb);
+        tab_bytes = (int)wpix_stage_tab_bytes(n_pos, eb);
         cs_bytes = kStageSfts * 16;
         d_bytes = kStageSfts * 32 * 8;
         w_bytes = kStageSfts * 4;

@@ -207,7 +207,7 @@ def test_pixel_lane_kernel_ragged(bsh, torch, ctx, n_sft, n_f0, margin, f0, side
     wl = synth.noise_workload(seed=1000 + n_sft + n_f0, n_sft=n_sft, n_f0=n_f0, margin=margin, f_band_start=f0,
                               n_pix_side=side, ap=(10.0, 40.0), P_days=(15.0, 31.0), n_t=3, topk=7)
     pk = oracle.peakgram(wl.rho)
-    want_n, _ = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL, want_wcount=False)
+    want_n, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
     ctx.set_option(bsh.BSH_OPT_KERNEL_FAMILY, bsh.BSH_FAMILY_PIXEL_LANE)
     for force_clamp in (False, True):
         ctx.set_option(bsh.BSH_OPT_FORCE_CLAMP, int(force_clamp))
@@ -215,6 +215,12 @@ def test_pixel_lane_kernel_ragged(bsh, torch, ctx, n_sft, n_f0, margin, f0, side
         assert ctx.stats()["kernel_variant"] // 1000 == 2, "the pixel-lane kernel did not run"
         assert np.array_equal(r["counts"], want_n), force_clamp
         check_unweighted_toplist(r["top"], want_n, 7)
+        r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED)
+        # (a clamped table of a 320-column slab does not fit two shared-memory stages: the template-lane kernel runs)
+        wide = force_clamp and n_f0 == 200
+        assert ctx.stats()["kernel_variant"] // 1000 == (1 if wide else 3), "the weighted pixel-lane kernel did not run"
+        assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=0), force_clamp
+        check_float_toplist(r["top"]["index"], want_w, 7)
 
 
 def test_pixel_lane_kernel_multiple_breaks(bsh, torch, ctx):
@@ -226,6 +232,10 @@ def test_pixel_lane_kernel_multiple_breaks(bsh, torch, ctx):
     r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED)
     assert ctx.stats()["kernel_variant"] // 1000 == 2
     assert np.array_equal(r["counts"], want_n)
+    _, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED)
+    assert ctx.stats()["kernel_variant"] // 1000 == 3
+    assert np.allclose(r["counts"], want_w, rtol=RTOL, atol=0)
 
 
 # ------------------------------------------------------------------------------------------------------------
