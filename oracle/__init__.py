@@ -52,6 +52,7 @@ def lib():
         _lib.orc_track_canonical.restype = C.c_int64
         _lib.orc_toplist.restype = C.c_int64
         _lib.orc_max_threads.restype = C.c_int
+        _lib.orc_median_bias.restype = C.c_double
     return _lib
 
 
@@ -97,6 +98,24 @@ def peakgram(rho: np.ndarray, rho_th: float = RHO_TH) -> np.ndarray:
     out = np.zeros((n, wpr), np.uint32)
     lib().orc_peakgram(C.c_void_p(rho.ctypes.data), C.c_int32(n), C.c_int32(k), C.c_float(rho_th),
                        C.c_void_p(out.ctypes.data), C.c_int32(wpr))
+    return out
+
+
+def median_bias(window: int = 101) -> float:
+    """E[median of `window` iid Exp(1) draws] = sum_{i=(window+1)/2}^{window} 1/i  (R-22; -> ln 2 for large windows)."""
+    return float(lib().orc_median_bias(C.c_int32(window)))
+
+
+def normalise(sft: np.ndarray, window: int = 101, bias=None) -> np.ndarray:
+    """PAPER.md Eq. (20)-(21), L167-L174: complex64 SFT bins [N, n_raw] -> normalised powers f32 [N, n_raw - window + 1]
+    (slab column k = raw bin k + (window - 1) / 2), noise estimated by the running median over `window` bins."""
+    sft = np.ascontiguousarray(sft, np.complex64)
+    n, n_raw = sft.shape
+    assert window % 2 == 1 and 1 <= window <= n_raw
+    b = np.float32(median_bias(window) if bias is None else bias)
+    out = np.zeros((n, n_raw - window + 1), np.float32)
+    lib().orc_normalise(C.c_void_p(sft.ctypes.data), C.c_int32(n), C.c_int32(n_raw), C.c_int32(window), C.c_float(b),
+                        C.c_void_p(out.ctypes.data))
     return out
 
 

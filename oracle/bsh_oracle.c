@@ -384,3 +384,61 @@ int64_t orc_toplist(const double *values, int64_t n, int64_t k, uint64_t *idx_ou
     free(p);
     return kk;
 }
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Front end, Eq. (20)-(21): complex SFT bins -> normalised power
+ *     rho_Jk = |x_Jk|^2 / <n_Jk>^2,
+ * "<n_Jk>^2 is usually estimated with a running median over a number of frequency bins (usually 101 bins are used)".
+ * The paper prints no formula for the estimate; reading R-22:
+ *   - input: n_raw complex bins per SFT (FP32 re, im interleaved, as SFT files store them); the slab column k is raw bin
+ *     k + h, h = (window - 1) / 2, so every output bin has a full window and there is no edge rule:
+ *     K = n_raw - window + 1 columns ("wing" bins on both sides are the caller's, as the SFT reader supplies them);
+ *   - power    p_q   = fl32(fl32(re re) + fl32(im im))                     (FP32, no FMA: the kernel's precision)
+ *   - median   med_k = the (h + 1)-th smallest of p_k .. p_{k + window - 1} (a selection: exact; NaN ranks above +inf)
+ *   - noise    n2_k  = fl32(med_k / bias)         bias = E[median of `window` iid Exp(1) draws] = sum_{i=h+1}^{window} 1/i
+ *                                                 (the median of exponential noise power is NOT its mean; for window -> inf
+ *                                                  the factor is ln 2.  Passed in as an FP32 number.)
+ *   - rho_k          = fl32(p_{k + h} / n2_k)
+ * Written as literally as that: copy the window, sort it, take the middle.
+ * ------------------------------------------------------------------------------------------------------- */
+double orc_median_bias(int32_t window)
+{
+    const int h = (window - 1) / 2;
+    double s = 0.0;
+    for (int i = window; i >= h + 1; --i) s += 1.0 / (double)i;      /* E of the (h+1)-th order statistic of Exp(1) */
+    return s;
+}
+
+static int cmp_float_nan_last(const void *a, const void *b)
+{
+    const float x = *(const float *)a, y = *(const float *)b;
+    const int xn = x != x, yn = y != y;
+    if (xn || yn) return xn - yn;                                   /* NaN above everything */
+    return (x > y) - (x < y);
+}
+
+void orc_normalise(const float *sft, int32_t n_sft, int32_t n_raw, int32_t window, float bias, float *rho)
+{
+    const int h = (window - 1) / 2;
+    const int K = n_raw - window + 1;
+    float *p = (float *)malloc(sizeof(float) * (size_t)n_raw);
+    float *win = (float *)malloc(sizeof(float) * (size_t)window);
+    for (int32_t J = 0; J < n_sft; ++J) {
+        const float *row = sft + 2 * (size_t)J * n_raw;
+        for (int q = 0; q < n_raw; ++q) {
+            const float re = row[2 * q], im = row[2 * q + 1];
+            const float rr = re * re;
+            const float ii = im * im;
+            p[q] = rr + ii;                                         /* |x|^2, Eq. (20) numerator */
+        }
+        for (int k = 0; k < K; ++k) {
+            memcpy(win, p + k, sizeof(float) * (size_t)window);
+            qsort(win, (size_t)window, sizeof(float), cmp_float_nan_last);
+            const float med = win[h];                               /* running median, L171 */
+            const float n2 = med / bias;                            /* <n>^2 estimate, Eq. (21) */
+            rho[(size_t)J * K + k] = p[k + h] / n2;                 /* Eq. (20) */
+        }
+    }
+    free(p);
+    free(win);
+}

@@ -425,6 +425,8 @@ int run_pass(bsh_ctx *ctx)
             p.cs = (const double2 *)c.d_cs.p;
             p.dpix = (const double *)ctx->dpix.p;
             p.split = (const unsigned char *)ctx->psplit.p;
+            p.one = 1u;
+            p.zero = 0u;
             p.A = (const double *)c.d_A.p;
             p.casa = (const double2 *)c.d_casa.p;
             p.n_pad = pd.n_pad; p.n_pos = pd.n_pos; p.n_chunks = pd.n_pad / kStageSfts; p.n_stages = pd.pix_stages;
@@ -784,6 +786,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         const int stride = weighted ? PosStage<kWarpsWeighted, 1, true>(pg.n_pos).stride
                                     : PosStage<kWarpsUnweighted, 2, false>(pg.n_pos).stride;
         const int budgets[3] = {112 * 1024, 112 * 1024, 224 * 1024};                          // 2 / 2 / 1 blocks per SM
+        const int pix_budgets[3] = {113 * 1024, 113 * 1024, 224 * 1024};                      // (228 KB - 1 KB per block) / 2
         pd.n_stages = 0;
         for (int b = 0; b < 3 && pd.n_stages < 2; ++b) pd.n_stages = std::min(kMaxStages, (budgets[b] - kPosHeader) / stride);
         pd.use_pos = pd.n_stages >= 2 && fam != BSH_FAMILY_WINDOW && !(mode & BSH_NAIVE);
@@ -792,11 +795,11 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         pd.n_oct = (pd.pos_groups + wpb - 1) / wpb;
         pd.pos_smem = kPosHeader + pd.n_stages * stride;
         // pixel-lane kernel (unweighted): pixels on the lanes pay off when most of the 32 lanes of a group are used
-        const PixStage ps(pg.n_pos);
+        const PixStage ps(pg.n_pos, pd.NW);
         pd.pix_stages = 0;
         const int hi_bytes = pix_hi_bytes(pd.NW, pd.HP);                                    // shared-memory high planes
         for (int b = 1; b < 3 && pd.pix_stages < 2; ++b)
-            pd.pix_stages = std::min(4, (budgets[b] - kPixHeader - hi_bytes) / ps.stride);      // (2..6 stages measure alike)
+            pd.pix_stages = std::min(4, (pix_budgets[b] - kPixHeader - hi_bytes) / ps.stride);  // (2..6 stages measure alike)
         pd.use_pix = !weighted && pd.pix_stages >= 2 && (lanes_ok || fam == BSH_FAMILY_PIXEL_LANE) &&
                      (fam == BSH_FAMILY_AUTO || fam == BSH_FAMILY_PIXEL_LANE) && !(mode & BSH_NAIVE);
         pd.pix_stages = std::max(1, std::min(pd.pix_stages, pd.n_pad / kStageSfts));
@@ -860,9 +863,9 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
             d_peak, words_per_row, sfts->n_sft, pd.n_pad, sfts->n_bins, pd.n_pos, pd.pos_off, pd.pos_s_zero,
             (uint4 *)ctx->ptab.p);
         count_launch(ctx);
-        TRY(ensure(ctx, ctx->psplit, (size_t)pd.n_pad * pd.n_pos * 12));
-        split_position_table_kernel<<<(unsigned)((n_ent + 255) / 256), 256, 0, ctx->stream>>>(
-            (const uint4 *)ctx->ptab.p, pd.n_pad, pd.n_pos, (unsigned char *)ctx->psplit.p);
+        TRY(ensure(ctx, ctx->psplit, (size_t)(pd.n_pad / kStageSfts) * (size_t)pix_stage_tab_bytes(pd.n_pos, pd.NW)));
+        pm_position_table_kernel<<<(unsigned)((n_ent + 255) / 256), 256, 0, ctx->stream>>>(
+            (const uint4 *)ctx->ptab.p, pd.n_pad, pd.n_pos, pd.NW, (unsigned char *)ctx->psplit.p);
         count_launch(ctx);
         const int64_t n_d = (int64_t)pd.n_pg * pd.n_pad * 32;
         dtable_pix_kernel<<<(unsigned)((n_d + 255) / 256), 256, 0, ctx->stream>>>(

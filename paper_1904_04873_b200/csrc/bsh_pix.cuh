@@ -29,7 +29,7 @@ namespace bsh {
 constexpr int kPixWarps = 8;                         // warps per block
 constexpr int kPixTpl = 2;                           // binary templates per thread
 constexpr int kPixTile = kPixWarps * kPixTpl;        // binary templates per block
-constexpr int kPixWarpScratch = 2 * kStageSfts * kPixTpl * 8 + kPixTpl * 32;   // two B buffers + template constants
+constexpr int kPixWarpScratch = kStageSfts * kPixTpl * 8 + kPixTpl * 32;       // B buffer of one stage + template constants
 constexpr int kPixHeader = 128 + kPixWarps * kPixWarpScratch;
 constexpr int kPixMid = 2;                           // high planes kept in registers (the other HP - 2 live in shared
                                                      // memory); 3 and 4 measured 2 % and 5 % slower on config 2
@@ -65,27 +65,35 @@ __global__ void __launch_bounds__(256) dtable_pix_kernel(const double *__restric
     dpix[t] = D;
 }
 
-// Split position table staged by the pixel-lane kernel: per stage of kStageSfts SFTs, first the (word 0, word 1) pairs
-// [kk][p] (8 bytes each), then the words 2 [kk][p] (4 bytes each).  The window of a position is then read with one
-// LDS.64 and one LDS.32 from two different arrays (12 bytes, 3 shared-memory wavefronts per warp) -- a 16-byte entry
-// would be fetched as one LDS.128 (4 wavefronts) whatever the source says, ptxas fuses adjacent reads.
-__global__ void __launch_bounds__(256) split_position_table_kernel(const uint4 *__restrict__ ptab, int n_pad, int n_pos,
-                                                                   unsigned char *__restrict__ split)
+// Position-major table staged by the pixel-lane kernel.  Per stage of kStageSfts SFTs, the RECORD of position p holds
+//   [kStageSfts] (word 0, word 1) pairs (8 bytes each), then for NW = 3 [kStageSfts] words 2 (4 bytes each), then 8 bytes
+//   of padding:  200 bytes (NW = 3) or 136 bytes (NW = 2).
+// Why: (i) the address of (SFT kk, position s) is  base + s * record + kk * 8  -- ONE multiply-add per triple (IMAD, on
+// the FMA pipe, which this kernel leaves idle) with the SFT part an instruction immediate, instead of the SEL + VIADD +
+// 2 LEA of an SFT-major table (all on the half-rate integer pipe that the LOP3 counters saturate); (ii) a window is read
+// as LDS.64 + LDS.32 (3 wavefronts; one LDS.128 would cost 4); (iii) 50 (34) words per record put the neighbouring
+// positions a warp reads (Eq. 34: pixels of a patch are less than a bin apart) into different banks.
+__host__ __device__ constexpr int pix_rec_bytes(int NW) { return NW >= 3 ? kStageSfts * 12 + 8 : kStageSfts * 8 + 8; }
+__host__ __device__ constexpr int pix_stage_tab_bytes(int n_pos, int NW) { return (n_pos * pix_rec_bytes(NW) + 15) & ~15; }
+
+__global__ void __launch_bounds__(256) pm_position_table_kernel(const uint4 *__restrict__ ptab, int n_pad, int n_pos, int NW,
+                                                                unsigned char *__restrict__ out)
 {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (int64_t)n_pad * n_pos) return;
     const int i = (int)(t / n_pos), p = (int)(t % n_pos);
     const uint4 e = ptab[t];
-    const int64_t stage_bytes = (int64_t)kStageSfts * n_pos * 12;
-    unsigned char *base = split + (int64_t)(i / kStageSfts) * stage_bytes;
+    const int rec = pix_rec_bytes(NW);
+    unsigned char *r = out + (int64_t)(i / kStageSfts) * pix_stage_tab_bytes(n_pos, NW) + (int64_t)p * rec;
     const int kk = i % kStageSfts;
-    reinterpret_cast<uint2 *>(base)[kk * n_pos + p] = make_uint2(e.x, e.y);
-    reinterpret_cast<uint32_t *>(base + (int64_t)kStageSfts * n_pos * 8)[kk * n_pos + p] = e.z;
+    reinterpret_cast<uint2 *>(r)[kk] = make_uint2(e.x, e.y);
+    if (NW >= 3) reinterpret_cast<uint32_t *>(r + kStageSfts * 8)[kk] = e.z;
+    if (kk == 0) *reinterpret_cast<uint2 *>(r + rec - 8) = make_uint2(0u, 0u);
 }
 
 struct PixParams {
     const uint4 *ptab;          // [n_pad][n_pos]  (fix-ups)
-    const unsigned char *split; // [n_pad / kStageSfts] stages of the split table (hot loop)
+    const unsigned char *split; // [n_pad / kStageSfts] stages of the position-major table (hot loop)
     const double2 *cs;          // [n_P][n_pad]  (cos, sin)(Omega_p t_i)
     const double *dpix;         // [n_pg][n_pad / 2][32][2]
     const double *A;            // [n_ap][n_P]
@@ -96,6 +104,7 @@ struct PixParams {
     int n_pg, n_aq, n_aq_tiles;
     double u0;                  // k_band0 + j0
     int off, s_max, s_zero;     // position coordinates (TrackConst)
+    unsigned int one, zero;     // 1 and 0 (run-time constants the compiler cannot fold, see pix_step)
     const Threshold *thr;
     RawCand *cand;
     unsigned int *cand_count;
@@ -105,9 +114,9 @@ struct PixParams {
 
 struct PixStage {
     int tab_bytes, cs_bytes, d_bytes, stride;
-    __device__ __host__ PixStage(int n_pos)
+    __device__ __host__ PixStage(int n_pos, int NW)
     {
-        tab_bytes = kStageSfts * n_pos * 12;
+        tab_bytes = pix_stage_tab_bytes(n_pos, NW);
         cs_bytes = kStageSfts * 16;
         d_bytes = kStageSfts * 32 * 8;
         stride = tab_bytes + cs_bytes + d_bytes;
@@ -142,47 +151,59 @@ __device__ __forceinline__ void pix_release(const PixParams &p, const PixStage &
 // Per-thread constants of the hot loop (the binary-term constants live in shared memory, only the fix-ups need them).
 struct PixConst {
     double u0, uL;
+    double magic;               // 1.5 2^52 + (off rounded down to even): the low word of fl(y + magic) is position - (off & 1);
+                                // an EVEN integer added to the rounding constant leaves the tie rule of R-1 unchanged
     int32_t off, s_max, s_zero;
+    uint32_t rec;               // bytes per record of the staged table (in a register, so that the address is one IMAD)
+    uint32_t s_zero_rel;        // s_zero - (off & 1)
+    uint32_t one, zero;         // 1 and 0, opaque to the compiler (kernel parameters)
 };
 
 // Position (table entry) to read for one (pixel, template, SFT) and the break flag (R-7): the all-zero position on a
-// break.  Unclamped geometry: the two magic-add results are compared as doubles (equal doubles <=> equal roundings),
-// which keeps the comparison on the FP64 pipe.
-template <bool CLAMP>
-__device__ __forceinline__ int32_t pix_position(const PixConst &k, double D, double B, bool &brk)
+// break.  Clamped geometry only (the unclamped hot path is pix_step below).
+__device__ __forceinline__ int32_t pix_position_clamped(const PixConst &k, double D, double B, bool &brk)
 {
     const double g = __dsub_rn(D, B);
     const double m0 = __dadd_rn(__dmul_rn(k.u0, g), kMagic);         // low word = round(fl(u0 g)), R-1
     const double mL = __dadd_rn(__dmul_rn(k.uL, g), kMagic);
-    int32_t s0 = k.off + __double2loint(m0);
-    if (CLAMP) {
-        int32_t sL = k.off + __double2loint(mL);
-        s0 = clamp_s(s0, k.s_max);
-        sL = clamp_s(sL, k.s_max);                       // equal after clamping => every bin reads 0
-        brk = s0 != sL;
-    } else {
-        brk = m0 != mL;
-    }
+    const int32_t s0 = clamp_s(k.off + __double2loint(m0), k.s_max);
+    const int32_t sL = clamp_s(k.off + __double2loint(mL), k.s_max); // equal after clamping => every bin reads 0
+    brk = s0 != sL;
     return brk ? k.s_zero : s0;
 }
 
-// Window of table index idx = stage row kk * n_pos + position: words 0, 1 from the pair array, word 2 from the word
-// array.
-template <int NW>
-__device__ __forceinline__ Win<NW> pix_load(const unsigned char *tab, int n_pos, int32_t idx)
+// Window of SFT KK of the stage from the record at shared-memory address `rec_addr`.
+template <int NW, int KK>
+__device__ __forceinline__ Win<NW> pix_load(uint32_t rec_addr)
 {
     Win<NW> w;
-    const uint2 lo = reinterpret_cast<const uint2 *>(tab)[idx];
-    w.x[0] = lo.x;
-    if (NW > 1) w.x[1 % NW] = lo.y;
-    if (NW > 2) w.x[2 % NW] = reinterpret_cast<const uint32_t *>(tab + kStageSfts * n_pos * 8)[idx];
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2+%3];" : "=r"(w.x[0]), "=r"(w.x[1 % NW]) : "r"(rec_addr), "n"(KK * 8));
+    if (NW > 2) asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(w.x[2 % NW]) : "r"(rec_addr), "n"(kStageSfts * 8 + KK * 4));
     return w;
 }
 
-// One SFT (slot K of the unrolled block of 32) for both templates of the thread.
+#ifndef BSH_PIX_SELMODE
+#define BSH_PIX_SELMODE 0
+#endif
+#ifndef BSH_PIX_BRKMODE
+#define BSH_PIX_BRKMODE 1
+#endif
+#if BSH_PIX_SELMODE == 1
+#define BSH_PIX_SEL_ASM "@p mad.lo.s32 lo, lo, %13, %6;\n\t"
+#else
+#define BSH_PIX_SEL_ASM "@p mov.b32 lo, %6;\n\t"
+#endif
+#if BSH_PIX_BRKMODE == 1
+#define BSH_PIX_BRK_ASM3 "@p mad.lo.u32 %3, %12, %7, %3;\n\t"
+#else
+#define BSH_PIX_BRK_ASM3 "@p or.b32 %3, %3, %7;\n\t"
+#endif
+
+// One SFT (slot K of the unrolled block of 32) for both templates of the thread.  base = shared-memory address of the
+// record of position (off & 1) of the stage (unclamped) or of position 0 (clamped).
 template <int K, int NW, int HP, bool CLAMP>
-__device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char *tab, int n_pos, const double2 *bpair,
-                                         const double2 *dpair, Counter<NW, kPixMid> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl])
+__device__ __forceinline__ void pix_step(const PixConst &k, uint32_t base, const double2 *bpair, const double2 *dpair,
+                                         Counter<NW, kPixMid> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl])
 {
     constexpr int kk = K % kStageSfts;
     const double2 d2 = dpair[(kk >> 1) * 32];
@@ -191,36 +212,61 @@ __device__ __forceinline__ void pix_step(const PixConst &k, const unsigned char 
     const double Bv[kPixTpl] = {b2.x, b2.y};
 #pragma unroll
     for (int r = 0; r < kPixTpl; ++r) {
-        int32_t s;                                       // table index: stage row + position
+        Win<NW> w;
         if (!CLAMP) {
-            // one predicate from the FP64 compare drives both the mask update (predicated OR) and the position select
+            // g = D - B, y at both band ends, rounding adds (the low word of m0 IS the table position), then ONE predicate
+            // from the FP64 compare (equal doubles <=> equal roundings) drives the break mask and the position select; the
+            // record address is one multiply-add.  6 FP64 + 1 FMA-pipe + 2 integer + 2 load instructions per triple.
             const double g = __dsub_rn(D, Bv[r]);
-            const double m0 = __dadd_rn(__dmul_rn(k.u0, g), kMagic);  // low word = round(fl(u0 g)) (R-1)
-            const double mL = __dadd_rn(__dmul_rn(k.uL, g), kMagic);
-            asm("{\n\t"
-                ".reg .pred p;\n\t"
-                "setp.neu.f64 p, %2, %3;\n\t"
-                "@p or.b32 %0, %0, %4;\n\t"
-                "selp.b32 %1, %5, %6, p;\n\t"
-                "}"
-                : "+r"(brk[r]), "=r"(s)
-                : "d"(m0), "d"(mL), "n"(1u << K), "r"(k.s_zero - k.off), "r"(__double2loint(m0)));
-            s += k.off + kk * n_pos;                     // position offset and stage row in one (warp-uniform) add
+            const double m0 = __dadd_rn(__dmul_rn(k.u0, g), k.magic);
+            const double mL = __dadd_rn(__dmul_rn(k.uL, g), k.magic);
+            // The select, the mask update and the address are written as multiply-adds with the run-time constant
+            // k.one (= 1): ptxas then issues them as IMAD on the FMA pipe instead of SEL / LOP3 / LEA on the integer
+            // pipe, which the LOP3 counters need.
+            if (NW > 2)
+                asm volatile("{\n\t"
+                             ".reg .pred p;\n\t"
+                             ".reg .b32 lo, hi, a;\n\t"
+                             "setp.neu.f64 p, %4, %5;\n\t"
+                             "mov.b64 {lo, hi}, %4;\n\t"
+                             BSH_PIX_SEL_ASM
+                             BSH_PIX_BRK_ASM3
+                             "mad.lo.s32 a, lo, %8, %9;\n\t"
+                             "ld.shared.v2.u32 {%0, %1}, [a+%10];\n\t"
+                             "ld.shared.u32 %2, [a+%11];\n\t"
+                             "}"
+                             : "=r"(w.x[0]), "=r"(w.x[1 % NW]), "=r"(w.x[2 % NW]), "+r"(brk[r])
+                             : "d"(m0), "d"(mL), "r"(k.s_zero_rel), "n"(1u << K), "r"(k.rec), "r"(base), "n"(kk * 8),
+                               "n"(kStageSfts * 8 + kk * 4), "r"(k.one), "r"(k.zero));
+            else
+                asm volatile("{\n\t"
+                             ".reg .pred p;\n\t"
+                             ".reg .b32 lo, hi, a;\n\t"
+                             "setp.neu.f64 p, %3, %4;\n\t"
+                             "mov.b64 {lo, hi}, %3;\n\t"
+                             "@p mov.b32 lo, %5;\n\t"
+                             "@p or.b32 %2, %2, %6;\n\t"
+                             "mad.lo.s32 a, lo, %7, %8;\n\t"
+                             "ld.shared.v2.u32 {%0, %1}, [a+%9];\n\t"
+                             "}"
+                             : "=r"(w.x[0]), "=r"(w.x[1 % NW]), "+r"(brk[r])
+                             : "d"(m0), "d"(mL), "r"(k.s_zero_rel), "n"(1u << K), "r"(k.rec), "r"(base), "n"(kk * 8));
         } else {
             bool b;
-            s = pix_position<CLAMP>(k, D, Bv[r], b) + kk * n_pos;
+            const int32_t s = pix_position_clamped(k, D, Bv[r], b);
             brk[r] |= b ? (1u << K) : 0u;
+            w = pix_load<NW, kk>(base + (uint32_t)s * k.rec);
         }
-        push<K, NW, kPixMid>(cnt[r], pix_load<NW>(tab, n_pos, s));
+        push<K, NW, kPixMid>(cnt[r], w);
     }
 }
 
 template <int K0, int NW, int HP, bool CLAMP, int... Ks>
-__device__ __forceinline__ void pix_half(const PixConst &k, const unsigned char *tab, int n_pos, const double2 *bpair,
-                                         const double2 *dpair, Counter<NW, kPixMid> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl],
+__device__ __forceinline__ void pix_half(const PixConst &k, uint32_t base, const double2 *bpair, const double2 *dpair,
+                                         Counter<NW, kPixMid> (&cnt)[kPixTpl], uint32_t (&brk)[kPixTpl],
                                          std::integer_sequence<int, Ks...>)
 {
-    (pix_step<K0 + Ks, NW, HP, CLAMP>(k, tab, n_pos, bpair, dpair, cnt, brk), ...);
+    (pix_step<K0 + Ks, NW, HP, CLAMP>(k, base, bpair, dpair, cnt, brk), ...);
 }
 
 #ifndef BSH_PIX_MINB
@@ -231,7 +277,7 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
 {
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);
-    const PixStage L(p.n_pos);
+    const PixStage L(p.n_pos, NW);
     int b = blockIdx.x;
     const int tile = b % p.n_aq_tiles;
     b /= p.n_aq_tiles;
@@ -239,8 +285,8 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
     const int pg = b / p.n_P;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     unsigned char *wscr = smem + 128 + warp * kPixWarpScratch;
-    double *bbuf = reinterpret_cast<double *>(wscr);                               // [2 halves][16 SFTs][2 templates]
-    double *tcst = reinterpret_cast<double *>(wscr + 2 * kStageSfts * kPixTpl * 8); // [2 templates][A, CA, SA, -]
+    double *bbuf = reinterpret_cast<double *>(wscr);                           // [16 SFTs][2 templates]
+    double *tcst = reinterpret_cast<double *>(wscr + kStageSfts * kPixTpl * 8); // [2 templates][A, CA, SA, -]
 
     // the warp's two binary templates (a_p, t_asc pairs of period ip); a missing one repeats the last real pair
     int ia[kPixTpl], it[kPixTpl];
@@ -282,6 +328,12 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
     kc.off = p.off;
     kc.s_max = p.s_max;
     kc.s_zero = p.s_zero;
+    kc.magic = kMagic + (double)(p.off & ~1);
+    kc.rec = (uint32_t)pix_rec_bytes(NW);
+    kc.s_zero_rel = (uint32_t)(p.s_zero - (p.off & 1));
+    kc.one = p.one;
+    kc.zero = p.zero;
+    const uint32_t rec_shift = CLAMP ? 0u : (uint32_t)(p.off & 1) * kc.rec;
 
     // Counters: 5 low planes (carry-save tree over a block of 32 SFTs) + kPixMid planes in registers; the HP - kPixMid
     // planes above live in shared memory, [plane][template][word][thread].  A register counter wraps at most once in
@@ -329,16 +381,16 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
             const double2 *cs = reinterpret_cast<const double2 *>(sp + L.tab_bytes);
             {   // binary terms of this stage: B = fl(A fl(fl(C CA) + fl(S SA)))  (R-5), one per lane
                 const double2 c = cs[lane >> 1];
-                bbuf[half * 32 + lane] = __dmul_rn(A_d, __dadd_rn(__dmul_rn(c.x, q_d.x), __dmul_rn(c.y, q_d.y)));
-                __syncwarp();
+                bbuf[lane] = __dmul_rn(A_d, __dadd_rn(__dmul_rn(c.x, q_d.x), __dmul_rn(c.y, q_d.y)));
+                __syncwarp();                            // (the previous stage's readers passed the __syncwarp of pix_release)
             }
-            const double2 *bpair = reinterpret_cast<const double2 *>(bbuf + half * 32);
+            const double2 *bpair = reinterpret_cast<const double2 *>(bbuf);
             const double2 *dpair = reinterpret_cast<const double2 *>(sp + L.tab_bytes + L.cs_bytes) + lane;
+            const uint32_t base = smem_u32(sp) + rec_shift;
             if (half == 0)
-                pix_half<0, NW, HP, CLAMP>(kc, sp, p.n_pos, bpair, dpair, cnt, brk,
-                                           std::make_integer_sequence<int, kStageSfts>{});
+                pix_half<0, NW, HP, CLAMP>(kc, base, bpair, dpair, cnt, brk, std::make_integer_sequence<int, kStageSfts>{});
             else
-                pix_half<kStageSfts, NW, HP, CLAMP>(kc, sp, p.n_pos, bpair, dpair, cnt, brk,
+                pix_half<kStageSfts, NW, HP, CLAMP>(kc, base, bpair, dpair, cnt, brk,
                                                     std::make_integer_sequence<int, kStageSfts>{});
             pix_release(p, L, smem, st, 2 * blk + half, lane, ip, pg);
             if (++st == p.n_stages) { st = 0; parity ^= 1u; }
