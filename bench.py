@@ -357,7 +357,7 @@ def main_ours(args, rank, local_rank, world):
 def kernel_name(variant: int, weighted: bool) -> str:
     fam = variant // 1000
     if weighted:
-        return {2: "stage1_weighted_pix_kernel", 1: "stage1_weighted_pos_kernel"}.get(fam, "stage1_weighted_kernel")
+        return {3: "stage1_weighted_pix_kernel", 1: "stage1_weighted_pos_kernel"}.get(fam, "stage1_weighted_kernel")
     return {2: "stage1_unweighted_pix_kernel", 1: "stage1_unweighted_pos_kernel"}.get(fam, "stage1_unweighted_kernel")
 
 

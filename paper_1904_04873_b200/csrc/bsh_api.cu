@@ -355,9 +355,9 @@ int dispatch_weighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p, i
 
 int dispatch_weighted_pix(bsh_ctx *ctx, const Pending &pd, const WpixParams &p, int grid)
 {
-    W_PIX_CASE(13, false)
+    W_PIX_CASE(15, false) W_PIX_CASE(8, false)
 #ifndef BSH_MINIMAL
-    W_PIX_CASE(13, true) W_PIX_CASE(8, false) W_PIX_CASE(8, true)
+    W_PIX_CASE(15, true) W_PIX_CASE(8, true)
 #endif
     return fail(ctx, BSH_EINVAL, "no weighted pixel-lane kernel for %d bytes clamp=%d", pd.wpix_nbytes, (int)pd.clamp);
 }
@@ -744,15 +744,18 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         pd.NW = 2;
         pd.tile_bins = (grid->n_f0 + 1) / 2;
     }
-    // weighted pixel-lane kernel (bsh_wpix.cuh): one pass over tiles of <= 91 bins (13 bytes of 7 bins; 8 bytes for <= 56)
+    // weighted pixel-lane kernel (bsh_wpix.cuh): one pass over tiles of <= 90 bins (15 bytes of 6 bins; 8 bytes for <= 48)
     pd.n_pg = (grid->n_pix + 31) / 32;
     const bool lanes_ok = 10 * grid->n_pix >= 6 * 32 * pd.n_pg;
     const int fam = ctx->opt_family;
     bool try_wpix = weighted && !(mode & BSH_NAIVE) && ((fam == BSH_FAMILY_AUTO && lanes_ok) || fam == BSH_FAMILY_PIXEL_LANE);
     if (try_wpix) {
-        const int n_tiles = (grid->n_f0 + 90) / 91;
+#ifndef BSH_WPIX_MAXBINS
+#define BSH_WPIX_MAXBINS 90
+#endif
+        const int n_tiles = (grid->n_f0 + BSH_WPIX_MAXBINS - 1) / BSH_WPIX_MAXBINS;
         const int tile = (grid->n_f0 + n_tiles - 1) / n_tiles;
-        const int nbytes = tile <= 56 ? 8 : 13, nw = nbytes == 8 ? 2 : 3;
+        const int nbytes = tile <= 48 ? 8 : 15, nw = nbytes == 8 ? 2 : 3;
         const TableGeometry tgw = table_geometry(sfts->n_sft, sfts->h_v_over_c, grid->n_P, grid->h_P, grid->n_ap, grid->h_ap,
                                                  grid->k_band0, sfts->k_slab0, grid->n_f0, sfts->n_bins, nw,
                                                  ctx->opt_force_clamp != 0);

@@ -4,11 +4,13 @@
 //
 // The method's work is one FP32 add per accumulation (template x SFT); this kernel is built so that little else is
 // issued:
-//   * thread = 1 pixel x 1 binary template x ALL f0 bins of the tile (up to 91 FP32 accumulators in registers);
+//   * thread = 1 pixel x 1 binary template x ALL f0 bins of the tile (up to 90 FP32 accumulators in registers);
 //     warp = one binary template x 32 neighbouring pixels; block = kWpixWarps templates of one period;
 //   * the window of peakgram bits a triple needs is read with ONE shared-memory load from a position table whose entries
-//     hold 7 bins per byte (bin j = bit j % 7 of byte j / 7): ptxas turns the seven `if (bit) acc += w` of a byte into one
-//     R2P (register byte -> 7 predicates) + 7 predicated FADD, no shifts, no masks;
+//     hold 6 bins per byte (bin j = bit j % 6 of byte j / 6): ptxas turns the six `if (bit) acc += w` of a byte into one
+//     R2P (register byte -> predicates P0..P5) + 6 predicated FADD, no shifts, no masks.  (7 bins per byte would need all
+//     seven predicate registers: ptxas then keeps one for the break flag and extracts every 7th bin with LOP3 + ISETP --
+//     measured 143 instead of 124 lane-instructions per triple; 15 bytes x 6 bins are exactly the 90 bins of a band);
 //   * the binary term B = A (C CA + S SA) of Eq. (15) (L102) is the same for the 32 lanes: lane l computes the one of SFT
 //     l & 15 of the stage and the warp shares them through shared memory; the hot loop has 6 FP64 operations per triple;
 //   * the position offset is folded into the rounding constant (an EVEN integer added to 1.5 2^52 leaves the tie rule of
@@ -33,8 +35,18 @@ namespace bsh {
 constexpr int kWpixWarps = BSH_WPIX_WARPS;           // warps (= binary templates) per block; one block per SM
 constexpr int kWpixHeader = 128 + kWpixWarps * kStageSfts * 8;   // mbarriers + one B buffer per warp
 
-// bins per byte-packed entry: NBYTES bytes of 7 bins
-__host__ __device__ constexpr int wpix_bins(int nbytes) { return 7 * nbytes; }
+// bins per byte-packed entry: NBYTES bytes of kWpixBits bins
+#ifndef BSH_WPIX_ROLL
+#define BSH_WPIX_ROLL 1
+#endif
+constexpr int kWpixBits = 6;
+#ifndef BSH_WPIX_SHIFT
+#define BSH_WPIX_SHIFT 1
+#endif
+constexpr int kWpixShift = BSH_WPIX_SHIFT;           // bin b of a byte sits in bit kWpixShift + b: with bits 1..6 every R2P has the
+                                                     // mask 0x7e (ptxas never takes bit 0 of a register into an R2P: it tests
+                                                     // it with LOP3 + ISETP), and P0 stays free for the break flag
+__host__ __device__ constexpr int wpix_bins(int nbytes) { return kWpixBits * nbytes; }
 __host__ __device__ constexpr int wpix_entry_bytes(int nbytes) { return nbytes <= 8 ? 8 : 16; }
 // The staged table is POSITION-MAJOR: the record of position p holds the entries of the stage's kStageSfts SFTs, plus one
 // entry of padding, so that (i) the address of (SFT kk, position s) is s * record + kk * entry -- one multiply-add per
@@ -44,8 +56,8 @@ __host__ __device__ constexpr int wpix_record_bytes(int eb) { return (kStageSfts
 // bytes of one stage of the table (n_pos records), rounded up to the 16 bytes a bulk copy moves
 __host__ __device__ constexpr int64_t wpix_stage_tab_bytes(int n_pos, int eb) { return ((int64_t)n_pos * wpix_record_bytes(eb) + 15) & ~(int64_t)15; }
 
-// 7-bins-per-byte position table: entry p of SFT i = the window STARTING at table position p (slab column p - off_table),
-// bin j in bit (j % 7) of byte (j / 7); bits outside [0, K), the padding SFTs and position s_zero are zero.
+// 6-bins-per-byte position table: entry p of SFT i = the window STARTING at table position p (slab column p - off_table),
+// bin j in bit (j % 6) of byte (j / 6); bits outside [0, K), the padding SFTs and position s_zero are zero.
 template <int EB>
 __global__ void __launch_bounds__(256) build_position7_table_kernel(const uint32_t *__restrict__ peak, int words_per_row,
                                                                     int n_sft, int n_pad, int n_bins, int n_pos,
@@ -70,11 +82,11 @@ __global__ void __launch_bounds__(256) build_position7_table_kernel(const uint32
     }
     uint32_t out[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
-    for (int q = 0; q < EB; ++q) {                       // byte q <- window bits [7 q, 7 q + 7)
-        const int b = 7 * q, w = b >> 5, s = b & 31;
+    for (int q = 0; q < EB; ++q) {                       // byte q <- window bits [6 q, 6 q + 6)
+        const int b = kWpixBits * q, w = b >> 5, s = b & 31;
         uint32_t bits = v[w] >> s;
-        if (s > 25 && w + 1 < 4) bits |= v[w + 1] << (32 - s);
-        out[q >> 2] |= (bits & 0x7Fu) << (8 * (q & 3));
+        if (s > 32 - kWpixBits && w + 1 < 4) bits |= v[w + 1] << (32 - s);
+        out[q >> 2] |= (bits & ((1u << kWpixBits) - 1u)) << (8 * (q & 3) + kWpixShift);
     }
     unsigned char *dst = tab + (int64_t)(i / kStageSfts) * wpix_stage_tab_bytes(n_pos, EB) + (int64_t)p * wpix_record_bytes(EB) +
                          (i % kStageSfts) * EB;
@@ -170,16 +182,18 @@ __device__ __forceinline__ Win7<NBYTES> load7(const unsigned char *entry)
     return w;
 }
 
-// acc[j] += wi for every bin j whose bit is set: bin j = bit (j % 7) of byte (j / 7)  (one R2P + 7 predicated FADD per byte)
+// acc[j] += wi for every bin j whose bit is set: bin j = bit (kWpixShift + j % 6) of byte (j / 6)  (one R2P + 6 predicated
+// FADD per byte).  (An inline-PTX form with the accumulators as read-write operands removes the ~2 register copies per
+// triple ptxas adds here, but costs 3 spill accesses per triple: measured 17.2 ms against 15.9 ms on config 2.)
 template <int NBYTES>
-__device__ __forceinline__ void accumulate7(float (&acc)[7 * NBYTES], const Win7<NBYTES> &x, float wi)
+__device__ __forceinline__ void accumulate7(float (&acc)[kWpixBits * NBYTES], const Win7<NBYTES> &x, float wi)
 {
 #pragma unroll
     for (int q = 0; q < NBYTES; ++q) {
         const uint32_t word = x.x[q >> 2];
 #pragma unroll
-        for (int b = 0; b < 7; ++b)
-            if (word & (1u << (8 * (q & 3) + b))) acc[7 * q + b] += wi;
+        for (int b = 0; b < kWpixBits; ++b)
+            if (word & (1u << (8 * (q & 3) + kWpixShift + b))) acc[kWpixBits * q + b] += wi;
     }
 }
 
@@ -192,7 +206,7 @@ struct WpixConst {
 // One SFT (slot K of the block of 32; KK = its row in the stage).
 template <int K, int NBYTES, bool CLAMP>
 __device__ __forceinline__ void wpix_step(const WpixConst &k, const unsigned char *tab, const double *bwarp,
-                                          const double2 *dpair, const float *wv, float (&acc)[7 * NBYTES], uint32_t &brk)
+                                          const double2 *dpair, const float *wv, float (&acc)[kWpixBits * NBYTES], uint32_t &brk)
 {
     constexpr int kk = K % kStageSfts;
     constexpr int EB = wpix_entry_bytes(NBYTES);
@@ -225,13 +239,13 @@ __device__ __forceinline__ void wpix_step(const WpixConst &k, const unsigned cha
 
 template <int K0, int NBYTES, bool CLAMP, int... Ks>
 __device__ __forceinline__ void wpix_half(const WpixConst &k, const unsigned char *tab, const double *bwarp,
-                                          const double2 *dpair, const float *wv, float (&acc)[7 * NBYTES], uint32_t &brk,
+                                          const double2 *dpair, const float *wv, float (&acc)[kWpixBits * NBYTES], uint32_t &brk,
                                           std::integer_sequence<int, Ks...>)
 {
     (wpix_step<K0 + Ks, NBYTES, CLAMP>(k, tab, bwarp, dpair, wv, acc, brk), ...);
 }
 
-// Exact window (7-bins-per-byte) of a (pixel, template, SFT) whose rounded shift differs between the two ends of the f0
+// Exact window (6-bins-per-byte) of a (pixel, template, SFT) whose rounded shift differs between the two ends of the f0
 // tile (R-7), from the global table: one break -> blend of the two neighbouring positions at the
 // break bin (estimated, then corrected on the canonical evaluation itself); otherwise every bin from its own position.
 template <int NBYTES, bool CLAMP>
@@ -255,7 +269,7 @@ __device__ __noinline__ Win7<NBYTES> exact_window7(const TrackConst &tc, const u
         while (j < tc.n_fj - 1 && tc.off + round_int(dmul(dadd(tc.u0, (double)j), g)) == s0) ++j;
         const Win7<NBYTES> a = load7<NBYTES>(entry7<EB>(tab, n_pos, i, s0));
         const Win7<NBYTES> b = load7<NBYTES>(entry7<EB>(tab, n_pos, i, sL));
-        const int pos = 8 * (j / 7) + (j % 7);           // bit position of bin j; bins >= j take the second window
+        const int pos = 8 * (j / kWpixBits) + (j % kWpixBits) + kWpixShift;   // bit position of bin j; bins >= j take the second window
 #pragma unroll
         for (int w = 0; w < NWORDS; ++w) {
             const int rel = pos - 32 * w;
@@ -269,7 +283,7 @@ __device__ __noinline__ Win7<NBYTES> exact_window7(const TrackConst &tc, const u
     for (int j = 0; j < tc.n_fj; ++j) {
         int32_t sj = tc.off + round_int(dmul(dadd(tc.u0, (double)j), g));
         sj = clamp_s(sj, tc.s_max);                      // identity in the unclamped geometry (proven range)
-        const int pos = 8 * (j / 7) + (j % 7);
+        const int pos = 8 * (j / kWpixBits) + (j % kWpixBits) + kWpixShift;
         const uint32_t word = reinterpret_cast<const uint32_t *>(entry7<EB>(tab, n_pos, i, sj))[pos >> 5];
         const uint32_t bit = (word >> (pos & 31)) & 1u;
 #pragma unroll
@@ -283,7 +297,7 @@ template <int NBYTES, bool CLAMP>
 __global__ void __launch_bounds__(32 * kWpixWarps, 1) stage1_weighted_pix_kernel(const WpixParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
-    constexpr int NB = 7 * NBYTES;
+    constexpr int NB = kWpixBits * NBYTES;
     constexpr int EB = wpix_entry_bytes(NBYTES);
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);
     const WpixStage L(p.n_pos, EB);
@@ -335,7 +349,11 @@ __global__ void __launch_bounds__(32 * kWpixWarps, 1) stage1_weighted_pix_kernel
     const int n_blocks = p.n_chunks >> 1;                // n_pad is a multiple of 32
     for (int blk = 0; blk < n_blocks; ++blk) {
         uint32_t brk = 0u;
+#if BSH_WPIX_ROLL
+#pragma unroll 1
+#else
 #pragma unroll
+#endif
         for (int half = 0; half < 2; ++half) {
             mbar_wait(&full[st], parity);
             const unsigned char *sp = smem + kWpixHeader + st * L.stride;
@@ -349,11 +367,17 @@ __global__ void __launch_bounds__(32 * kWpixWarps, 1) stage1_weighted_pix_kernel
             const double2 *dpair = reinterpret_cast<const double2 *>(sp + L.tab_bytes + L.cs_bytes) + lane;
             const float *wv = reinterpret_cast<const float *>(sp + L.tab_bytes + L.cs_bytes + L.d_bytes);
             const unsigned char *tab = sp + (p.off & 1) * wpix_record_bytes(EB);
+#if BSH_WPIX_ROLL
+            uint32_t brk16 = 0u;                         // one copy of the stage's code for both halves of the block
+            wpix_half<0, NBYTES, CLAMP>(kc, tab, bwarp, dpair, wv, acc, brk16, std::make_integer_sequence<int, kStageSfts>{});
+            brk |= brk16 << (kStageSfts * half);
+#else
             if (half == 0)
                 wpix_half<0, NBYTES, CLAMP>(kc, tab, bwarp, dpair, wv, acc, brk, std::make_integer_sequence<int, kStageSfts>{});
             else
                 wpix_half<kStageSfts, NBYTES, CLAMP>(kc, tab, bwarp, dpair, wv, acc, brk,
                                                      std::make_integer_sequence<int, kStageSfts>{});
+#endif
             wpix_release(p, L, smem, st, 2 * blk + half, lane, ip, pg);
             if (++st == p.n_stages) { st = 0; parity ^= 1u; }
         }
