@@ -107,6 +107,7 @@ typedef struct {
     int32_t  grid_blocks;        /* of the accumulation kernel                                                     */
     int64_t  launches;           /* kernels launched by this context since creation                                */
     float    host_tables_ms;     /* host time spent building cos/sin tables in the last call (0 when cached)       */
+    float    frontend_ms;        /* bsh_normalise_peakgram kernel                                                  */
 } bsh_stats;
 
 /* On-chip peak rates of the context's device, MEASURED by bsh_measure_peaks() with microbenchmark kernels (32 warps
@@ -142,6 +143,24 @@ int bsh_measure_peaks(bsh_ctx *ctx, bsh_peaks *h_out);             /* ~50 ms of 
  * beyond ceil(n_bins / 32) are zeroed.  Asynchronous. */
 int bsh_build_peakgram(bsh_ctx *ctx, const float *d_rho, int32_t n_sft, int32_t n_bins, int64_t rho_row_stride,
                        float rho_th, uint32_t *d_peak, int32_t words_per_row);
+
+/* Front end (L167-L176, Eq. 20-21): complex SFT bins -> normalised powers -> peakgram, one fused kernel.
+ *     rho_Jk = |x_Jk|^2 / <n_Jk>^2,   <n_Jk>^2 = running median of |x|^2 over `window` bins / median_bias   (reading R-22)
+ *   d_sft        [n_sft][sft_row_stride] complex bins, FP32 (re, im) interleaved (8 bytes per bin, 8-byte aligned),
+ *                sft_row_stride >= n_raw (in complex elements); raw bin q of row J is d_sft[2 (J stride + q)], [.. + 1]
+ *   n_raw        raw bins per row = K + window - 1: slab column k is raw bin k + (window - 1) / 2, so every column has a
+ *                full window (the caller supplies (window - 1) / 2 wing bins on each side; there is no edge rule)
+ *   window       odd, 1 <= window <= n_raw <= 2048; the paper uses 101
+ *   median_bias  E[median of `window` iid Exp(1) draws] (bsh_median_bias(window); -> ln 2 for large windows): the median of
+ *                exponentially distributed noise power is not its mean, dividing by it makes <rho> = 1 in noise (L439)
+ *   d_rho        [n_sft][rho_row_stride] FP32 normalised powers, K = n_raw - window + 1 columns written per row; may be NULL
+ *   d_peak       [n_sft][words_per_row] bit-packed (rho > rho_th), layout as bsh_build_peakgram; may be NULL (not both)
+ * Arithmetic (FP32, each operation rounded once, no FMA): p = fl(fl(re re) + fl(im im)); med = the ((window + 1) / 2)-th
+ * smallest p of the window (exact selection; NaN ranks above +inf); n2 = fl(med / bias); rho = fl(p / n2).  Asynchronous. */
+int bsh_normalise_peakgram(bsh_ctx *ctx, const float *d_sft, int32_t n_sft, int32_t n_raw, int64_t sft_row_stride,
+                           int32_t window, float median_bias, float rho_th, float *d_rho, int64_t rho_row_stride,
+                           uint32_t *d_peak, int32_t words_per_row);
+double bsh_median_bias(int32_t window);    /* sum_{i = (window + 1) / 2}^{window} 1 / i; host function                     */
 
 /* Stage 1 (L223, L241-L247): number count of every template of `grid` along its Eq. (15) track through the
  * peakgram, and the per-patch toplist (L217, L225).

@@ -14,7 +14,7 @@ BSH_OPT_KERNEL_FAMILY, BSH_OPT_FORCE_CLAMP, BSH_OPT_PIXELS_PER_THREAD = 1, 2, 3
 BSH_FAMILY_AUTO, BSH_FAMILY_PIXEL_LANE, BSH_FAMILY_TEMPLATE_LANE, BSH_FAMILY_WINDOW = 0, 1, 2, 3
 
 EXPORTS = ["bsh_version", "bsh_create", "bsh_destroy", "bsh_last_error", "bsh_get_stats", "bsh_set_option",
-           "bsh_measure_peaks", "bsh_build_peakgram",
+           "bsh_measure_peaks", "bsh_build_peakgram", "bsh_normalise_peakgram", "bsh_median_bias",
            "bsh_stage1_hough", "bsh_stage1_launch", "bsh_stage1_collect", "bsh_stage2_power", "bsh_search_patch_host",
            "bsh_template_index", "bsh_template_decode"]
 
@@ -42,7 +42,7 @@ class Stats(C.Structure):
                 ("stage1_select_ms", C.c_float), ("stage2_ms", C.c_float), ("n_templates", C.c_int64),
                 ("n_accumulations", C.c_int64), ("n_candidates", C.c_int64), ("threshold", C.c_double),
                 ("n_passes", C.c_int32), ("kernel_variant", C.c_int32), ("threads_per_block", C.c_int32),
-                ("grid_blocks", C.c_int32), ("launches", C.c_int64), ("host_tables_ms", C.c_float)]
+                ("grid_blocks", C.c_int32), ("launches", C.c_int64), ("host_tables_ms", C.c_float), ("frontend_ms", C.c_float)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -71,6 +71,7 @@ def library():
         lib.bsh_last_error.restype = C.c_char_p
         lib.bsh_template_index.restype = C.c_uint64
         lib.bsh_template_decode.restype = None
+        lib.bsh_median_bias.restype = C.c_double
         for name in EXPORTS:
             getattr(lib, name)                       # fail loudly on a missing symbol
         _lib = lib
@@ -93,6 +94,10 @@ class _Problem:
                           n_P=a["P"].shape[0], h_P=a["P"].ctypes.data, n_tasc=a["tf"].shape[0],
                           h_tasc_frac=a["tf"].ctypes.data)
         self.d_w = d_w
+
+
+def median_bias(window: int = 101) -> float:
+    return float(library().bsh_median_bias(C.c_int32(window)))
 
 
 def template_index(wl, pix, ia, ip, it, j) -> int:
@@ -152,6 +157,23 @@ class Context:
                                                 C.c_int64(d_rho.stride(0)), C.c_float(rho_th), C.c_void_p(out.data_ptr()),
                                                 C.c_int32(out.shape[1])))
         return out
+
+    def normalise_peakgram(self, d_sft, window: int = 101, bias=None, rho_th: float = 1.6, want_rho=True, want_peak=True):
+        """d_sft: CUDA complex64 [N, n_raw] (row stride = d_sft.stride(0)).  Returns (d_rho float32 [N, K] or None,
+        d_peak int32 [N, ceil(K / 32)] or None), K = n_raw - window + 1 (front end, Eq. 20-21 + L176)."""
+        torch = self.torch
+        assert d_sft.is_cuda and d_sft.dtype == torch.complex64 and d_sft.dim() == 2 and d_sft.stride(1) == 1
+        n, n_raw = d_sft.shape
+        k = n_raw - window + 1
+        b = median_bias(window) if bias is None else bias
+        d_rho = torch.empty((n, k), dtype=torch.float32, device=d_sft.device) if want_rho else None
+        d_peak = torch.empty((n, (k + 31) // 32), dtype=torch.int32, device=d_sft.device) if want_peak else None
+        self._check(self.lib.bsh_normalise_peakgram(
+            self._ctx, C.c_void_p(d_sft.data_ptr()), C.c_int32(n), C.c_int32(n_raw), C.c_int64(d_sft.stride(0)),
+            C.c_int32(window), C.c_float(b), C.c_float(rho_th), C.c_void_p(d_rho.data_ptr() if want_rho else None),
+            C.c_int64(k), C.c_void_p(d_peak.data_ptr() if want_peak else None),
+            C.c_int32(d_peak.shape[1] if want_peak else 0)))
+        return d_rho, d_peak
 
     def stage1_launch(self, d_peak, wl, mode=BSH_UNWEIGHTED, topk=None, d_w=None, counts_full=None):
         pb = _Problem(wl, d_w)

@@ -19,6 +19,7 @@
 #include "bsh_pix.cuh"
 #include "bsh_wpix.cuh"
 #include "bsh_peaks.cuh"
+#include "bsh_frontend.cuh"
 
 using namespace bsh;
 
@@ -80,11 +81,12 @@ struct bsh_ctx {
     DevBuf wtab, w_pad, stats, thr, dtab, nvec, cand, cand_count, keys, tmp_cands, dtab2, nvec2, ptab, dpos, dpix, psplit, tab7;
     DevBuf h_rho, h_w, h_peak, h_top;                  // device staging of bsh_search_patch_host
     unsigned int *pinned_count = nullptr;
-    cudaEvent_t ev[10] = {};
+    cudaEvent_t ev[12] = {};
     Pending pend;
     int opt_family = BSH_FAMILY_AUTO, opt_force_clamp = 0, opt_pixels_per_thread = 0;   // bsh_set_option
     DevBuf peak_samples;
     bsh_stats st = {};
+    bool have_front = false;
     bool have_pk = false, have_setup = false, have_kernel = false, have_select = false, have_s2 = false;
     float kernel_ms_extra = 0.f;
 };
@@ -629,6 +631,7 @@ int bsh_get_stats(bsh_ctx *ctx, bsh_stats *out)
         ctx->st.stage1_kernel_ms = ms + ctx->kernel_ms_extra;
     if (ctx->have_select && cudaEventElapsedTime(&ms, ctx->ev[4], ctx->ev[5]) == cudaSuccess) ctx->st.stage1_select_ms = ms;
     if (ctx->have_s2 && cudaEventElapsedTime(&ms, ctx->ev[6], ctx->ev[7]) == cudaSuccess) ctx->st.stage2_ms = ms;
+    if (ctx->have_front && cudaEventElapsedTime(&ms, ctx->ev[10], ctx->ev[11]) == cudaSuccess) ctx->st.frontend_ms = ms;
     *out = ctx->st;
     return BSH_OK;
 }
@@ -707,6 +710,43 @@ int bsh_build_peakgram(bsh_ctx *ctx, const float *d_rho, int32_t n_sft, int32_t 
     CK(cudaGetLastError());
     CK(cudaEventRecord(ctx->ev[9], ctx->stream));
     ctx->have_pk = true;
+    return BSH_OK;
+}
+
+double bsh_median_bias(int32_t window)
+{
+    if (window < 1) return 0.0;
+    double s = 0.0;                                       // expectation of the middle order statistic of `window` Exp(1) draws
+    for (int i = (window + 1) / 2; i <= window; ++i) s += 1.0 / (double)i;
+    return s;
+}
+
+int bsh_normalise_peakgram(bsh_ctx *ctx, const float *d_sft, int32_t n_sft, int32_t n_raw, int64_t sft_row_stride,
+                           int32_t window, float median_bias, float rho_th, float *d_rho, int64_t rho_row_stride,
+                           uint32_t *d_peak, int32_t words_per_row)
+{
+    if (!ctx) return BSH_EINVAL;
+    if (!d_sft || (!d_rho && !d_peak) || n_sft < 1 || n_raw < 1 || sft_row_stride < n_raw)
+        return fail(ctx, BSH_EINVAL, "bsh_normalise_peakgram: bad arguments");
+    if (window < 1 || (window & 1) == 0 || window > n_raw) return fail(ctx, BSH_EINVAL, "window must be odd and <= n_raw");
+    if (n_raw > kFrontMaxRaw) return fail(ctx, BSH_EINVAL, "n_raw > %d: split the band", kFrontMaxRaw);
+    if (!(median_bias > 0.f)) return fail(ctx, BSH_EINVAL, "median_bias must be positive");
+    if ((uintptr_t)d_sft % 8 != 0) return fail(ctx, BSH_EINVAL, "d_sft must be 8-byte aligned");
+    const int K = n_raw - window + 1;
+    if (d_rho && rho_row_stride < K) return fail(ctx, BSH_EINVAL, "rho_row_stride < n_raw - window + 1");
+    if (d_peak && (int64_t)words_per_row * 32 < K) return fail(ctx, BSH_ESMALL, "words_per_row * 32 < n_raw - window + 1");
+    const DeviceGuard device_guard(ctx->device);
+    int n2 = 32;
+    while (n2 < n_raw) n2 <<= 1;
+    const size_t smem = (size_t)n2 * 8 + (size_t)n_raw * 8;
+    CK(cudaEventRecord(ctx->ev[10], ctx->stream));
+    normalise_peakgram_kernel<<<(unsigned)n_sft, kFrontThreads, smem, ctx->stream>>>(
+        (const float2 *)d_sft, n_raw, sft_row_stride, window, median_bias, rho_th, d_rho, rho_row_stride, d_peak,
+        words_per_row, n2);
+    count_launch(ctx);
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(ctx->ev[11], ctx->stream));
+    ctx->have_front = true;
     return BSH_OK;
 }
 

@@ -261,6 +261,29 @@ class Config4:
 
     def deposit(self, bins_per_injection: List[np.ndarray]) -> np.ndarray:
         """rho = |x|^2 after adding A*exp(i*phi_i) to bin bins[inj][i] of SFT i (R-17); bins < 0 or >= K skip."""
+        re, im = self.deposit_bins(bins_per_injection)
+        return np.ascontiguousarray(re * re + im * im, np.float32)
+
+    def raw_bins(self, bins_per_injection: List[np.ndarray], window: int = 101, noise_sigma: float = 1.0) -> np.ndarray:
+        """Complex SFT bins as the front end takes them (Eq. 19-20): the K slab bins of deposit_bins()
+        plus (window - 1) / 2 wing bins of fresh noise on each side, every SFT scaled by a seeded log-normal noise
+        amplitude sqrt(S_J) (a non-stationary detector) and by a gentle slope across the band (a coloured spectrum) --
+        what the running-median normalisation has to take out again.  complex64 [N, K + window - 1]."""
+        re, im = self.deposit_bins(bins_per_injection)
+        n, k = re.shape
+        h = (window - 1) // 2
+        rng = _rng(self.base.seed, 4242)
+        wing = rng.standard_normal((n, 2, h, 2)) * math.sqrt(0.5)
+        x = np.empty((n, k + 2 * h), np.complex128)
+        x[:, h:h + k] = re + 1j * im
+        x[:, :h] = wing[:, 0, :, 0] + 1j * wing[:, 0, :, 1]
+        x[:, h + k:] = wing[:, 1, :, 0] + 1j * wing[:, 1, :, 1]
+        amp = np.exp(0.5 * noise_sigma * rng.standard_normal(n))[:, None]
+        slope = 1.0 + 0.2 * (np.arange(k + 2 * h)[None, :] / (k + 2 * h) - 0.5)
+        return np.ascontiguousarray(x * amp * np.sqrt(slope), np.complex64)
+
+    def deposit_bins(self, bins_per_injection: List[np.ndarray]):
+        """(re, im) [N, K] f64 after adding A*exp(i*phi_i) to bin bins[inj][i] of SFT i (R-17); bins outside the slab skip."""
         re, im = self.re.copy(), self.im.copy()
         amp = math.sqrt(self.amp2)
         n, k = re.shape
@@ -270,7 +293,7 @@ class Config4:
             ok = (bins >= 0) & (bins < k)
             re[rows[ok], bins[ok]] += amp * np.cos(inj.phases[ok])
             im[rows[ok], bins[ok]] += amp * np.sin(inj.phases[ok])
-        return np.ascontiguousarray(re * re + im * im, np.float32)
+        return re, im
 
 
 def config4(seed: int = 4, n_patches: int = 10) -> Config4:
@@ -353,6 +376,16 @@ def noise_workload(seed: int, n_sft: int, n_f0: int, margin: int, f_band_start: 
     alpha, delta = patch_pixels(a0, d0, pixel_size(t_sft, f_band_start, 1.0), n_pix_side, n_pix_side)
     return _finish(f"noise-{seed}", seed, t_sft, starts, v, f_band_start, n_f0 / t_sft, margin, rho, w, alpha, delta,
                    np.asarray(ap, np.float64), np.asarray(P_days, np.float64) * DAY, tasc_fractions(n_t), topk)
+
+
+def raw_sft_bins(seed: int, n_sft: int, n_raw: int, noise_sigma: float = 2.0) -> np.ndarray:
+    """Noise-only complex SFT bins for the front end (Eq. 19-21): unit complex Gaussian bins times a seeded
+    log-normal per-SFT amplitude (orders of magnitude apart) and a slope across the band.  complex64 [N, n_raw]."""
+    rng = _rng(seed, 4243)
+    x = (rng.standard_normal((n_sft, n_raw)) + 1j * rng.standard_normal((n_sft, n_raw))) * math.sqrt(0.5)
+    amp = np.exp(0.5 * noise_sigma * rng.standard_normal(n_sft))[:, None]
+    slope = 1.0 + 0.3 * (np.arange(n_raw)[None, :] / max(n_raw, 1) - 0.5)
+    return np.ascontiguousarray(x * amp * np.sqrt(slope), np.complex64)
 
 
 def tie_workload() -> Workload:

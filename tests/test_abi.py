@@ -33,12 +33,25 @@ def test_library_is_built_for_sm_100a_with_tma_and_fp64_no_fma():
     assert "sm_100a" in out
     sass = subprocess.run(["cuobjdump", "-sass", path], capture_output=True, text=True).stdout
     kernels = sass.split("Function : ")
-    acc = [k for k in kernels if k.startswith("_ZN3bsh24stage1_unweighted_kernel") or k.startswith("_ZN3bsh22stage1_weighted_kernel")]
-    assert acc
-    for k in acc:
-        assert "UBLKCP" in k, "accumulation kernels stage their chunks with TMA bulk copies"
-        assert "DFMA" not in k, "track arithmetic must not contract to FMA (DESIGN.md R-5)"
-        assert "DMUL" in k and "DADD" in k and "LOP3" in k
+    # every accumulation-kernel family: the ones the bench runs (pixel-lane, weighted pixel-lane), the template-lane
+    # position-table kernels and the funnel-shift fallbacks
+    families = {"stage1_unweighted_pix_kernel": "LOP3", "stage1_weighted_pix_kernel": "FADD",
+                "stage1_unweighted_pos_kernel": "LOP3", "stage1_weighted_pos_kernel": "FADD",
+                "stage1_unweighted_kernel": "LOP3", "stage1_weighted_kernel": "FADD"}
+    for name, count_op in families.items():
+        acc = [k for k in kernels if k.startswith(f"_ZN3bsh{len(name)}{name}")]
+        assert acc, name
+        for k in acc:
+            assert "UBLKCP" in k, f"{name}: accumulation kernels stage their tables with TMA bulk copies"
+            assert "DFMA" not in k, f"{name}: track arithmetic must not contract to FMA (DESIGN.md R-5)"
+            assert "DMUL" in k and "DADD" in k and count_op in k, name
+    pix = [k for k in kernels if k.startswith("_ZN3bsh28stage1_unweighted_pix_kernel")]
+    assert all("LDS.64" in k for k in pix), "pixel-lane kernel: 8-byte window reads from the position-major table"
+    assert all("DSETP" in k for k in pix if "Lb0EEE" in k.split("\n")[0]), "unclamped pixel-lane kernel: FP64 break predicate"
+    wpix = [k for k in kernels if k.startswith("_ZN3bsh26stage1_weighted_pix_kernel")]
+    assert all("R2P" in k for k in wpix), "weighted pixel-lane kernel: predicates of a byte of bins set by one R2P"
+    front = [k for k in kernels if k.startswith("_ZN3bsh25normalise_peakgram_kernel")]
+    assert front and all("FMUL" in k and "FADD" in k for k in front), "front end: |x|^2 as rounded FP32 products and sum (R-22)"
 
 
 def test_template_index_roundtrip_and_order():

@@ -73,6 +73,30 @@ def check_float_toplist(idx_got, values_ref, k, rtol=RTOL):
         assert abs(values_ref[i] - cut) <= rtol * abs(cut), (i, values_ref[i], cut)
 
 
+def check_toplist_complete(torch, d_counts, top, k, weighted):
+    """No better template was dropped: against the FULL dump of the ranking statistic (on the device, O(n), library ops
+    only): every template above the cut value is in the toplist, and the entries AT the cut are the lowest indices
+    (unweighted: exactly; weighted: inside the 1e-5 band of the k-th value)."""
+    vals = top["wcount"] if weighted else top["count"]
+    cut = vals[k - 1]
+    d_cut = torch.tensor(cut, dtype=d_counts.dtype, device=d_counts.device)
+    if weighted:
+        lo, hi = cut * (1 - RTOL), cut * (1 + RTOL)
+        above = torch.nonzero(d_counts > hi).flatten().cpu().numpy()
+        assert set(above.tolist()) <= set(int(i) for i in top["index"])
+        n_ge = int((d_counts >= lo).sum())
+        assert n_ge >= k
+        got = d_counts[torch.from_numpy(top["index"].astype(np.int64)).to(d_counts.device)].cpu().numpy()
+        assert np.array_equal(got, vals) and np.all(got >= lo)
+    else:
+        above = torch.nonzero(d_counts > d_cut).flatten().cpu().numpy()
+        n_above = above.size
+        assert n_above < k and n_above == int((vals > cut).sum())
+        assert np.array_equal(np.sort(top["index"][:n_above].astype(np.int64)), above)
+        at = torch.nonzero(d_counts == d_cut).flatten()[:k - n_above].cpu().numpy()
+        assert np.array_equal(top["index"][n_above:k].astype(np.int64), at)
+
+
 # ------------------------------------------------------------------------------------------------------------
 # peakgram
 # ------------------------------------------------------------------------------------------------------------
@@ -309,10 +333,13 @@ def test_config2_full_size_unweighted(bsh, torch, ctx):
     assert np.array_equal(rn["counts"], r["counts"])
     assert np.array_equal(rn["top"]["index"], r["top"]["index"])
     # noise statistics of the full dump: Binomial(2000, e^-1.6) up to the sample's peak fraction
-    p_hat = np.unpackbits(oracle.peakgram(wl.rho).view(np.uint8)).sum() / (wl.n_sft * wl.n_bins)
-    # (p_hat has a sampling error of sqrt(p(1-p)/(N K)) = 7e-4, i.e. 1.4 counts: allow 4 sigma)
-    assert abs(r["counts"].mean() - wl.n_sft * p_hat) < 6.0
-    assert abs(r["counts"].std() / math.sqrt(wl.n_sft * p_hat * (1 - p_hat)) - 1) < 0.05
+    # The mean count over all templates is a WEIGHTED mean of this realisation's peakgram bits (each (row, column) weighted
+    # by how many tracks visit it; a track visits one of >= n_f0 = 90 columns of a row), so it scatters around the closed
+    # form N e^-1.6 (L439) with a standard deviation of at most sqrt(N p (1 - p) / n_f0) = 1.9 counts: allow 4 sigma.
+    p = math.exp(-1.6)
+    assert abs(r["counts"].mean() - wl.n_sft * p) < 4.0 * math.sqrt(wl.n_sft * p * (1 - p) / wl.n_f0)
+    assert abs(r["counts"].std() / math.sqrt(wl.n_sft * p * (1 - p)) - 1) < 0.05
+    check_toplist_complete(torch, torch.from_numpy(r["counts"]).cuda(), r["top"], wl.topk, weighted=False)
 
 
 def test_config2_full_size_weighted(bsh, torch, ctx):
@@ -327,14 +354,24 @@ def test_config3_full_size_weighted(bsh, torch, ctx):
 
 
 def test_config3_full_size_unweighted_toplist(bsh, torch, ctx):
+    """All 1.66e9 integer counts dumped: the toplist is complete (nothing above the cut is missing, ties at the cut are
+    the lowest indices), its entries equal the oracle's re-score, and a seeded sample of the dump equals the oracle."""
     wl = synth.config3()
-    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=wl.topk, full=False)
+    d_rho, d_w = dev(torch, wl.rho), dev(torch, wl.w)
+    d_peak = ctx.build_peakgram(d_rho, 1.6)
+    d_counts = torch.full((wl.n_templates,), -7, dtype=torch.int32, device="cuda")
+    d_top, n_top = ctx.stage1_hough(d_peak, wl, mode=bsh.BSH_UNWEIGHTED, topk=wl.topk, d_w=d_w, counts_full=d_counts)
+    top = ctx.records(d_top, n_top)
     pk = oracle.peakgram(wl.rho)
-    n_o, w_o, _ = oracle.score(wl, r["top"]["index"], peak=pk, w=wl.w)
-    assert np.array_equal(r["top"]["count"], n_o)
-    assert np.all(np.diff(r["top"]["count"].astype(np.int64)) <= 0)
-    ties = np.diff(r["top"]["count"].astype(np.int64)) == 0
-    assert np.all(np.diff(r["top"]["index"].astype(np.int64))[ties] > 0)
+    n_o, w_o, _ = oracle.score(wl, top["index"], peak=pk, w=wl.w)
+    assert np.array_equal(top["count"], n_o)
+    assert np.all(np.diff(top["count"].astype(np.int64)) <= 0)
+    ties = np.diff(top["count"].astype(np.int64)) == 0
+    assert np.all(np.diff(top["index"].astype(np.int64))[ties] > 0)
+    check_toplist_complete(torch, d_counts, top, wl.topk, weighted=False)
+    idx = np.random.default_rng(321).integers(0, wl.n_templates, 1500)
+    n_s, _, _ = oracle.score(wl, idx.astype(np.uint64), peak=pk, w=None)
+    assert np.array_equal(d_counts[torch.from_numpy(idx).cuda()].cpu().numpy(), n_s)
 
 
 # ------------------------------------------------------------------------------------------------------------
@@ -348,11 +385,17 @@ def test_config4_signal_recovery(bsh, torch, ctx):
         bins.append(oracle.track(wl_p, inj.pix, inj.ia, inj.ip, inj.it, inj.j, mode=oracle.DIRECT))
     rho = c4.deposit(bins)
     pk = oracle.peakgram(rho)
+    rng = np.random.default_rng(44)
     for inj in c4.injections:
         wl = c4.patch_workload(inj.patch, rho)
-        r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=1000, full=False)
+        r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=1000, full=True)
         want = oracle.encode_index(wl, inj.pix, inj.ia, inj.ip, inj.it, inj.j)
         assert int(r["top"]["index"][0]) == want, inj.patch
+        # completeness of the toplist against the full dump, and a sample of the dump against the oracle
+        check_toplist_complete(torch, torch.from_numpy(r["counts"]).cuda(), r["top"], 1000, weighted=False)
+        idx = rng.integers(0, wl.n_templates, 200)
+        n_s, _, _ = oracle.score(wl, idx.astype(np.uint64), peak=pk, w=None)
+        assert np.array_equal(r["counts"][idx], n_s)
         n_o, _, _ = oracle.score(wl, r["top"]["index"], peak=pk, w=None)
         assert np.array_equal(r["top"]["count"], n_o)
         p_sig = 0.29568
@@ -369,7 +412,10 @@ def test_config4_signal_recovery(bsh, torch, ctx):
 # ------------------------------------------------------------------------------------------------------------
 def test_config5_two_streams(bsh, torch):
     c5 = synth.config5()
-    patches = [0, 100, 255, 17]
+    # 16 of the 256 patches: every declination band of the 16 x 16 tiling (index = i_alpha * 16 + i_delta), varying alpha
+    patches = [((5 * d + 3) % 16) * 16 + d for d in range(16)]
+    assert len({p % 16 for p in patches}) == 16 and 100 not in patches
+    patches[6] = 100
     streams = [torch.cuda.Stream(), torch.cuda.Stream()]
     ctxs = [bsh.Context(0, stream=s) for s in streams]
     d_rho = dev(torch, c5.base.rho)
@@ -406,12 +452,19 @@ def test_config5_two_streams(bsh, torch):
         assert np.allclose(recs["wcount"], w_o, rtol=RTOL, atol=0)
         assert np.allclose(recs["power"], p_o, rtol=RTOL, atol=0)
         assert np.all(np.diff(recs["power"]) <= 0)
-    # same patch on one stream gives the same toplist
-    with torch.cuda.stream(streams[0]):
-        d_top, n_top = ctxs[0].stage1_hough(d_peak, wls[100], topk=1000, d_w=keep[100])
-        ctxs[0].stage2_power(d_rho, wls[100], d_top, n_top, d_w=keep[100], sort_by_power=True)
-    torch.cuda.synchronize()
-    assert np.array_equal(ctxs[0].records(d_top, n_top), ctxs[0].records(results[100][0], 1000))
+    # same patch on one stream gives the same toplist; with the full dump: the streamed toplists are complete
+    for ip in (100, patches[0], patches[15]):
+        with torch.cuda.stream(streams[0]):
+            d_counts = torch.full((wls[ip].n_templates,), -7, dtype=torch.int32, device="cuda")
+            d_top, n_top = ctxs[0].stage1_hough(d_peak, wls[ip], topk=1000, d_w=keep[ip], counts_full=d_counts)
+            top1 = ctxs[0].records(d_top, n_top).copy()
+            ctxs[0].stage2_power(d_rho, wls[ip], d_top, n_top, d_w=keep[ip], sort_by_power=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(ctxs[0].records(d_top, n_top), ctxs[0].records(results[ip][0], 1000))
+        check_toplist_complete(torch, d_counts, top1, 1000, weighted=False)
+        idx = np.random.default_rng(ip).integers(0, wls[ip].n_templates, 200)
+        n_s, _, _ = oracle.score(wls[ip], idx.astype(np.uint64), peak=pk, w=None)
+        assert np.array_equal(d_counts[torch.from_numpy(idx).cuda()].cpu().numpy(), n_s)
     for c in ctxs:
         c.close()
 
@@ -432,6 +485,25 @@ def test_search_patch_host_end_to_end(bsh, torch, ctx):
     assert np.all(np.diff(recs["power"]) <= 0)
     st = ctx.stats()
     assert st["launches"] > 0 and st["n_templates"] == 1620
+
+
+@pytest.mark.parametrize("weighted", [False, True])
+def test_search_patch_host_at_config2_size(bsh, torch, ctx, weighted):
+    """The call `e2e` times in bench.py, at the size it is timed at: record by record against the device-buffer path,
+    and every record against the oracle's re-score."""
+    wl = synth.config2()
+    mode = bsh.BSH_WEIGHTED if weighted else bsh.BSH_UNWEIGHTED
+    recs, n_top = ctx.search_patch_host(wl.rho, wl.w, wl, mode=mode, topk=wl.topk)
+    assert n_top == wl.topk
+    r = gpu_stage1(bsh, torch, ctx, wl, mode, topk=wl.topk, full=False)
+    ctx.stage2_power(r["d_rho"], wl, r["d_top"], r["n_top"], d_w=r["d_w"], sort_by_power=True)
+    dev_recs = ctx.records(r["d_top"], r["n_top"])
+    assert np.array_equal(recs, dev_recs)
+    n_o, w_o, p_o = oracle.score(wl, recs["index"], peak=oracle.peakgram(wl.rho), rho=wl.rho, w=wl.w)
+    assert np.array_equal(recs["count"], n_o)
+    assert np.allclose(recs["wcount"], w_o, rtol=RTOL, atol=0)
+    assert np.allclose(recs["power"], p_o, rtol=RTOL, atol=0)
+    assert np.all(np.diff(recs["power"]) <= 0)
 
 
 def test_ties_round_to_even_on_the_gpu(bsh, torch, ctx):

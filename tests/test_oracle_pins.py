@@ -423,3 +423,102 @@ def test_ties_round_to_even():
     pk = oracle.peakgram(wl.rho)
     cnt, _ = oracle.stage1(wl, pk, None, mode=oracle.CANONICAL)
     assert cnt[0] == int(np.sum(want % 2 == 0))
+
+
+# ------------------------------------------------------------------------------------------------------------
+# Front end: running-median normalisation, Eq. (20)-(21), reading R-22
+# ------------------------------------------------------------------------------------------------------------
+def test_normalise_hand_worked_example():
+    g = _read_golden("running_median_example.txt")
+    amp = np.array([float(v) for v in g["amplitudes"].split()])
+    want = np.array([float(v) for v in g["rho"].split()])
+    x = amp.astype(np.complex64)[None, :]
+    got = oracle.normalise(x, window=int(g["window"]))
+    assert np.allclose(got[0], want, rtol=3e-7, atol=0)
+    assert abs(oracle.median_bias(3) - float(g["bias"])) < 1e-15
+    # the same powers carried by the imaginary part, or split between the two, give the same rho (|x|^2 = re^2 + im^2)
+    assert np.array_equal(oracle.normalise((1j * amp).astype(np.complex64)[None, :], window=3), got)
+    x2 = (amp * (0.6 + 0.8j)).astype(np.complex64)[None, :]
+    assert np.allclose(oracle.normalise(x2, window=3), got, rtol=1e-6)
+    # peak bits of the example: only column 1 exceeds 1.0; none exceeds the paper's 1.6
+    assert oracle.peakgram(got, 1.0)[0, 0] == 0b0010 and oracle.peakgram(got, 1.6)[0, 0] == 0
+
+
+def test_median_bias_closed_form_and_monte_carlo():
+    from fractions import Fraction
+    g = _read_golden("running_median_example.txt")
+    assert abs(oracle.median_bias(101) - float(g["median_bias_101"])) < 1e-14
+    for w in (1, 3, 5, 21, 101):
+        exact = sum(Fraction(1, i) for i in range((w + 1) // 2, w + 1))       # E of the middle order statistic of Exp(1)
+        assert abs(oracle.median_bias(w) - float(exact)) < 1e-14
+    assert oracle.median_bias(1) == 1.0                                      # window of one bin: the mean itself
+    assert 0 < oracle.median_bias(100001) - float(g["ln2"]) < 1e-5          # large-window limit ln 2
+    rng = np.random.default_rng(7)
+    med = np.median(rng.standard_exponential((200000, 101)), axis=1)
+    assert abs(med.mean() - oracle.median_bias(101)) < 5 * med.std() / math.sqrt(med.size)
+
+
+@pytest.mark.parametrize("n,n_raw,window", [(3, 101, 101), (5, 150, 101), (4, 40, 3), (2, 64, 1), (6, 352, 101), (2, 33, 33)])
+def test_normalise_equals_numpy_sliding_median(n, n_raw, window):
+    """np.median over numpy's sliding_window_view is a library routine, not the oracle's copy-sort-pick loop."""
+    x = synth.raw_sft_bins(11, n, n_raw)
+    got = oracle.normalise(x, window)
+    re, im = x.real.astype(np.float32), x.imag.astype(np.float32)
+    p = re * re + im * im
+    med = np.median(np.lib.stride_tricks.sliding_window_view(p, window, axis=1), axis=-1).astype(np.float32)
+    h = (window - 1) // 2
+    want = p[:, h:n_raw - h] / (med / np.float32(oracle.median_bias(window)))
+    assert got.shape == (n, n_raw - window + 1)
+    assert np.array_equal(got, want)
+
+
+def test_normalise_statistics_scale_invariance_and_lines():
+    n, k, window = 400, 200, 101
+    x = synth.raw_sft_bins(5, n, k + window - 1, noise_sigma=3.0)            # per-SFT noise levels spread over e^{+-4.5}
+    rho = oracle.normalise(x, window).astype(np.float64)
+    # PAPER.md L439: normalised noise power is Exp(1): mean 1, P(rho > 1.6) = e^{-1.6}.  The 101-bin median estimate has a
+    # relative scatter of ~1/sqrt(101 ln^2 2 ...) ~ 10 %, which biases <1/median> up by ~1 %: allow 3 %.
+    assert abs(rho.mean() - 1.0) < 0.03
+    frac = (rho > 1.6).mean()
+    assert abs(frac - math.exp(-1.6)) < 0.01
+    # every SFT is normalised on its own: per-row means agree although the raw levels differ by orders of magnitude
+    raw_level = (np.abs(x) ** 2).mean(axis=1)
+    assert raw_level.max() / raw_level.min() > 1e2
+    assert np.abs(rho.mean(axis=1) - 1.0).max() < 0.35
+    # scaling one SFT by a power of two changes nothing, bit for bit (every operation scales exactly)
+    y = x.copy()
+    y[3] *= np.complex64(2.0 ** 7)
+    y[9] *= np.complex64(2.0 ** -5)
+    assert np.array_equal(oracle.normalise(y, window), oracle.normalise(x, window))
+    # a narrow spectral line (3 bins, 1000 x the noise power) stands out and barely moves the noise estimate around it:
+    z = x.copy()
+    z[:, 150:153] *= np.complex64(math.sqrt(1000.0))
+    rz = oracle.normalise(z, window).astype(np.float64)
+    h = (window - 1) // 2
+    assert (rz[:, 150 - h:153 - h] > 20).mean() > 0.96                       # P(1000 Exp(1) > 20) = 0.98
+    far = np.r_[0:40]                                                        # columns whose windows do not contain the line
+    assert np.array_equal(rz[:, far], rho[:, far])
+    near = np.r_[60:99]                                                      # windows containing the 3 line bins: the median
+    ratio = rho[:, near] / rz[:, near]                                       # moves up by ~3 order statistics of 101 (~6 %)
+    assert 1.0 <= ratio.min() and ratio.mean() < 1.12
+
+
+def test_normalise_special_values():
+    """Constant power -> rho = bias (|x|^2 / (|x|^2 / bias)); zero median -> inf / NaN; NaN bins rank last."""
+    b = np.float32(oracle.median_bias(5))
+    x = np.full((1, 9), 3.0 + 4.0j, np.complex64)                            # |x|^2 = 25 everywhere
+    got = oracle.normalise(x, 5)
+    assert np.allclose(got, b, rtol=2e-7)
+    x = np.zeros((1, 7), np.complex64)
+    x[0, 3] = 2.0
+    got = oracle.normalise(x, 5)                                             # medians are 0: 0/0 = NaN, 4/0 = inf
+    assert np.isnan(got[0, 0]) and np.isinf(got[0, 1]) and np.isnan(got[0, 2])
+    assert oracle.peakgram(got)[0, 0] == 0b010                               # NaN > 1.6 is false, inf > 1.6 is true
+    x = (np.arange(1, 8) + 0j).astype(np.complex64)[None, :]
+    x[0, 1] = np.nan
+    got = oracle.normalise(x, 3)
+    # windows of |x|^2: (1, NaN, 9) -> median 9; (NaN, 9, 16) -> 16; (9, 16, 25) -> 16; ...
+    b3 = np.float32(oracle.median_bias(3))
+    assert np.isnan(got[0, 0])                                               # centre bin is the NaN
+    assert np.isclose(got[0, 1], np.float32(9.0) / (np.float32(16.0) / b3))
+    assert np.isclose(got[0, 2], np.float32(16.0) / (np.float32(16.0) / b3))
