@@ -38,7 +38,8 @@ class _Problem(C.Structure):
                 ("t_search_mid", C.c_double), ("k_slab0", C.c_int64), ("n_bins", C.c_int32), ("k_band0", C.c_int64),
                 ("n_f0", C.c_int32), ("n_pix", C.c_int32), ("alpha", C.c_void_p), ("delta", C.c_void_p),
                 ("n_ap", C.c_int32), ("ap", C.c_void_p), ("n_P", C.c_int32), ("P", C.c_void_p),
-                ("n_tasc", C.c_int32), ("tasc_frac", C.c_void_p)]
+                ("n_tasc", C.c_int32), ("tasc_frac", C.c_void_p),
+                ("n_ecc", C.c_int32), ("ecosw", C.c_void_p), ("esinw", C.c_void_p)]
 
 
 _lib = None
@@ -70,15 +71,23 @@ class Problem:
     def __init__(self, wl):
         self.arrays = dict(t_mid=_f64(wl.t_mid), v_over_c=_f64(wl.v_over_c), alpha=_f64(wl.alpha),
                            delta=_f64(wl.delta), ap=_f64(wl.ap), P=_f64(wl.P), tasc_frac=_f64(wl.tasc_frac))
+        ecw, esw = getattr(wl, "ecosw", None), getattr(wl, "esinw", None)
+        n_ecc = 0 if ecw is None else len(ecw)
+        if n_ecc:
+            self.arrays.update(ecosw=_f64(ecw), esinw=_f64(esw))
+            assert self.arrays["ecosw"].shape == self.arrays["esinw"].shape == (n_ecc,)
         a = self.arrays
         self.c = _Problem(n_sft=a["t_mid"].shape[0], t_sft=float(wl.t_sft), t_mid=a["t_mid"].ctypes.data,
                           v_over_c=a["v_over_c"].ctypes.data, t_search_mid=float(wl.t_search_mid),
                           k_slab0=int(wl.k_slab0), n_bins=int(wl.n_bins), k_band0=int(wl.k_band0), n_f0=int(wl.n_f0),
                           n_pix=a["alpha"].shape[0], alpha=a["alpha"].ctypes.data, delta=a["delta"].ctypes.data,
                           n_ap=a["ap"].shape[0], ap=a["ap"].ctypes.data, n_P=a["P"].shape[0], P=a["P"].ctypes.data,
-                          n_tasc=a["tasc_frac"].shape[0], tasc_frac=a["tasc_frac"].ctypes.data)
+                          n_tasc=a["tasc_frac"].shape[0], tasc_frac=a["tasc_frac"].ctypes.data,
+                          n_ecc=n_ecc, ecosw=a["ecosw"].ctypes.data if n_ecc else None,
+                          esinw=a["esinw"].ctypes.data if n_ecc else None)
         self.n_sft = self.c.n_sft
-        self.shape = (self.c.n_pix, self.c.n_ap, self.c.n_P, self.c.n_tasc, self.c.n_f0)
+        self.n_ecc = n_ecc
+        self.shape = (self.c.n_pix, self.c.n_ap, self.c.n_P, self.c.n_tasc, max(1, n_ecc), self.c.n_f0)
         self.n_templates = int(np.prod([int(s) for s in self.shape]))
 
     @property
@@ -119,12 +128,13 @@ def normalise(sft: np.ndarray, window: int = 101, bias=None) -> np.ndarray:
     return out
 
 
-def track(wl, pix, ia, ip, it, j, mode=CANONICAL, with_aux=False):
-    """Slab column per SFT for one template (Eq. 15).  aux = x (DIRECT) or y (CANONICAL), the unrounded values."""
+def track(wl, pix, ia, ip, it, j, mode=CANONICAL, with_aux=False, ie=0):
+    """Slab column per SFT for one template (Eq. 15; Eq. 14 when the workload has eccentricity pairs, `ie` = pair index).
+    aux = x (DIRECT) or y (CANONICAL), the unrounded values."""
     pb = Problem(wl)
     k = np.zeros(pb.n_sft, np.int64)
     aux = np.zeros(pb.n_sft, np.float64)
-    lib().orc_track(pb.ref, C.c_int(mode), C.c_int(pix), C.c_int(ia), C.c_int(ip), C.c_int(it), C.c_int(j),
+    lib().orc_track(pb.ref, C.c_int(mode), C.c_int(pix), C.c_int(ia), C.c_int(ip), C.c_int(it), C.c_int(ie), C.c_int(j),
                     C.c_void_p(k.ctypes.data), C.c_void_p(aux.ctypes.data))
     return (k, aux) if with_aux else k
 
@@ -181,14 +191,17 @@ def toplist(values, k: int) -> np.ndarray:
 
 
 def decode_index(wl, idx):
+    """(pix, ia, ip, it, j) for a circular grid, (pix, ia, ip, it, ie, j) when the workload has eccentricity pairs."""
     pb = Problem(wl)
-    out = np.zeros(5, np.int32)
+    out = np.zeros(6, np.int32)
     lib().orc_decode_index(pb.ref, C.c_uint64(int(idx)), C.c_void_p(out.ctypes.data))
-    return tuple(int(x) for x in out)
+    t = tuple(int(x) for x in out)
+    return t if pb.n_ecc else t[:4] + t[5:]
 
 
-def encode_index(wl, pix, ia, ip, it, j) -> int:
-    return ((((pix * len(wl.ap) + ia) * len(wl.P) + ip) * len(wl.tasc_frac) + it) * wl.n_f0 + j)
+def encode_index(wl, pix, ia, ip, it, j, ie=0) -> int:
+    n_ecc = 1 if getattr(wl, "ecosw", None) is None else len(wl.ecosw)
+    return (((((pix * len(wl.ap) + ia) * len(wl.P) + ip) * len(wl.tasc_frac) + it) * n_ecc + ie) * wl.n_f0 + j)
 
 
 # --- significances (R-10): derived from independent Bernoulli(p) / Exp(1) terms; constant within a patch -------

@@ -7,6 +7,8 @@
  *
  *   peakgram      PAPER.md L176  (section IV.A): bin -> 1 if rho > rho_th (= 1.6), else 0
  *   track         PAPER.md L102  Eq. (15):  f(t) = f0 + f0 v(t).n/c - f0 a_p Omega cos[Omega (t - t_asc)],
+ *                 and, for small eccentricity (ELL1), L95-L98 Eq. (14): the two further terms
+ *                 - f0 a_p Omega e cos(omega) cos[2 Omega (t - t_asc)] + f0 a_p Omega e sin(omega) sin[2 Omega (t - t_asc)],
  *                 Omega = 2 pi / P (L61), a_p in seconds (L70), t_asc range Eq. (35),
  *                 f0 lattice delta f = 1/T_c (Eq. 33); bin = round((f - f_slab_start) T)  (BASELINE.json)
  *   stage 1       PAPER.md L223  (section IV.C): number count n = weighted sum of 1s and 0s along the track
@@ -52,7 +54,13 @@ typedef struct {
     int32_t n_ap;   const double *ap;          /* seconds */
     int32_t n_P;    const double *P;           /* seconds */
     int32_t n_tasc; const double *tasc_frac;   /* t_asc = t_search_mid + frac * P, frac in [-1/2, 1/2) */
+    int32_t n_ecc;  const double *ecosw, *esinw;  /* SURVEY NEXT-3, Eq. (14): [n_ecc] pairs (e cos omega, e sin omega);
+                                                  n_ecc = 0: circular orbits, Eq. (15) */
 } orc_problem;
+
+static inline int n_ecc_eff(const orc_problem *pb) { return pb->n_ecc > 0 ? pb->n_ecc : 1; }
+static inline double ecc_k(const orc_problem *pb, int ie) { return pb->n_ecc > 0 ? pb->ecosw[ie] : 0.0; }
+static inline double ecc_h(const orc_problem *pb, int ie) { return pb->n_ecc > 0 ? pb->esinw[ie] : 0.0; }
 
 enum { ORC_DIRECT = 0, ORC_CANONICAL = 1 };
 
@@ -85,7 +93,7 @@ void orc_peakgram(const float *rho, int32_t n_sft, int32_t n_bins, float rho_th,
  * Returns the slab column (may lie outside [0, K): such an SFT contributes nothing, R-6).
  * If x_out != NULL it receives x, the unrounded bin coordinate (for near-tie flagging).
  * ------------------------------------------------------------------------------------------------------- */
-int64_t orc_track_direct(const orc_problem *pb, int pix, int ia, int ip, int it, int j, int i, double *x_out)
+int64_t orc_track_direct(const orc_problem *pb, int pix, int ia, int ip, int it, int ie, int j, int i, double *x_out)
 {
     const double T = pb->t_sft;
     const double alpha = pb->alpha[pix], delta = pb->delta[pix];
@@ -97,7 +105,12 @@ int64_t orc_track_direct(const orc_problem *pb, int pix, int ia, int ip, int it,
     const double Omega = 2.0 * M_PI / P;                                /* L61 */
     const double t_asc = pb->t_search_mid + pb->tasc_frac[it] * P;      /* Eq. (35) */
     const double a_p = pb->ap[ia];
-    const double f = f0 + f0 * v_dot_n - f0 * a_p * Omega * cos(Omega * (pb->t_mid[i] - t_asc));   /* Eq. (15) */
+    double f = f0 + f0 * v_dot_n - f0 * a_p * Omega * cos(Omega * (pb->t_mid[i] - t_asc));         /* Eq. (15) */
+    if (pb->n_ecc > 0) {                                                /* Eq. (14): the O(e) terms of the ELL1 model */
+        const double ecw = pb->ecosw[ie], esw = pb->esinw[ie];
+        f = f - f0 * a_p * Omega * ecw * cos(2.0 * Omega * (pb->t_mid[i] - t_asc))
+              + f0 * a_p * Omega * esw * sin(2.0 * Omega * (pb->t_mid[i] - t_asc));
+    }
     const double f_slab = (double)pb->k_slab0 / T;
     const double x = (f - f_slab) * T;
     if (x_out) *x_out = x;
@@ -109,6 +122,10 @@ int64_t orc_track_direct(const orc_problem *pb, int pix, int ia, int ip, int it,
  *   y = u_j * g,  u_j = k_band0 + j  (= f0_j * T, an exact integer),  g = v.n/c - a_p Omega cos[Omega(t - t_asc)]
  * and cos[Omega(t - t_asc)] = cos(Omega t) cos(Omega t_asc) + sin(Omega t) sin(Omega t_asc).
  * Every operation below is one rounded FP64 operation in the order written.
+ * Eccentric tracks (Eq. 14; R-23): g = v.n/c - A [cos phi + k cos 2 phi - h sin 2 phi], k = e cos(omega),
+ * h = e sin(omega), phi = Omega (t - t_asc), with sin phi = S CA - C SA and the double angle from cos phi, sin phi:
+ * cos 2 phi = cos^2 phi - sin^2 phi, sin 2 phi = 2 sin phi cos phi (rounded +, -, * only; k = h = 0 gives Eq. (15)
+ * bit for bit).
  * ------------------------------------------------------------------------------------------------------- */
 static void unit_vector(double alpha, double delta, double n[3])
 {
@@ -127,13 +144,28 @@ static double canon_D(const double *v, const double n[3])
     return ab + c;
 }
 
-static int64_t canon_bin(const orc_problem *pb, double D, double A, double C, double S, double CA, double SA, int j,
-                         double *y_out)
+static int64_t canon_bin(const orc_problem *pb, double D, double A, double C, double S, double CA, double SA, double k,
+                         double h, int j, double *y_out)
 {
     const double cc = C * CA;
     const double ss = S * SA;
     const double cphi = cc + ss;
-    const double B = A * cphi;
+    double bracket = cphi;
+    if (k != 0.0 || h != 0.0) {
+        const double sc = S * CA;
+        const double cs = C * SA;
+        const double sphi = sc - cs;
+        const double c2a = cphi * cphi;
+        const double s2a = sphi * sphi;
+        const double cos2 = c2a - s2a;
+        const double two_s = 2.0 * sphi;
+        const double sin2 = two_s * cphi;
+        const double kc = k * cos2;
+        const double hs = h * sin2;
+        const double E = kc - hs;
+        bracket = cphi + E;
+    }
+    const double B = A * bracket;
     const double g = D - B;
     const double u = (double)(pb->k_band0 + j);
     const double y = u * g;
@@ -142,7 +174,7 @@ static int64_t canon_bin(const orc_problem *pb, double D, double A, double C, do
     return (pb->k_band0 - pb->k_slab0) + j + r;
 }
 
-int64_t orc_track_canonical(const orc_problem *pb, int pix, int ia, int ip, int it, int j, int i, double *y_out)
+int64_t orc_track_canonical(const orc_problem *pb, int pix, int ia, int ip, int it, int ie, int j, int i, double *y_out)
 {
     double n[3];
     unit_vector(pb->alpha[pix], pb->delta[pix], n);
@@ -155,33 +187,35 @@ int64_t orc_track_canonical(const orc_problem *pb, int pix, int ia, int ip, int 
     const double ta = pb->t_search_mid + fp;
     const double arg_t = Omega * pb->t_mid[i];
     const double arg_a = Omega * ta;
-    return canon_bin(pb, D, A, cos(arg_t), sin(arg_t), cos(arg_a), sin(arg_a), j, y_out);
+    return canon_bin(pb, D, A, cos(arg_t), sin(arg_t), cos(arg_a), sin(arg_a), ecc_k(pb, ie), ecc_h(pb, ie), j, y_out);
 }
 
 /* one full track (all SFTs) of one template, either mode */
-void orc_track(const orc_problem *pb, int mode, int pix, int ia, int ip, int it, int j, int64_t *k_out, double *aux_out)
+void orc_track(const orc_problem *pb, int mode, int pix, int ia, int ip, int it, int ie, int j, int64_t *k_out,
+               double *aux_out)
 {
     for (int i = 0; i < pb->n_sft; ++i) {
         double aux;
-        k_out[i] = (mode == ORC_DIRECT) ? orc_track_direct(pb, pix, ia, ip, it, j, i, &aux)
-                                        : orc_track_canonical(pb, pix, ia, ip, it, j, i, &aux);
+        k_out[i] = (mode == ORC_DIRECT) ? orc_track_direct(pb, pix, ia, ip, it, ie, j, i, &aux)
+                                        : orc_track_canonical(pb, pix, ia, ip, it, ie, j, i, &aux);
         if (aux_out) aux_out[i] = aux;
     }
 }
 
-/* template linear index (R-11): f0 fastest */
-static inline uint64_t tmpl_index(const orc_problem *pb, int pix, int ia, int ip, int it, int j)
+/* template linear index (R-11): f0 fastest, then the eccentricity pair (one value when the grid is circular) */
+static inline uint64_t tmpl_index(const orc_problem *pb, int pix, int ia, int ip, int it, int ie, int j)
 {
-    return ((((uint64_t)pix * pb->n_ap + ia) * pb->n_P + ip) * pb->n_tasc + it) * pb->n_f0 + j;
+    return (((((uint64_t)pix * pb->n_ap + ia) * pb->n_P + ip) * pb->n_tasc + it) * n_ecc_eff(pb) + ie) * pb->n_f0 + j;
 }
 
-void orc_decode_index(const orc_problem *pb, uint64_t idx, int32_t *out5)
+void orc_decode_index(const orc_problem *pb, uint64_t idx, int32_t *out6)
 {
-    out5[4] = (int32_t)(idx % pb->n_f0);   idx /= pb->n_f0;     /* j   */
-    out5[3] = (int32_t)(idx % pb->n_tasc); idx /= pb->n_tasc;   /* it  */
-    out5[2] = (int32_t)(idx % pb->n_P);    idx /= pb->n_P;      /* ip  */
-    out5[1] = (int32_t)(idx % pb->n_ap);   idx /= pb->n_ap;     /* ia  */
-    out5[0] = (int32_t)idx;                                     /* pix */
+    out6[5] = (int32_t)(idx % pb->n_f0);      idx /= pb->n_f0;        /* j   */
+    out6[4] = (int32_t)(idx % n_ecc_eff(pb)); idx /= n_ecc_eff(pb);   /* ie  */
+    out6[3] = (int32_t)(idx % pb->n_tasc);    idx /= pb->n_tasc;      /* it  */
+    out6[2] = (int32_t)(idx % pb->n_P);       idx /= pb->n_P;         /* ip  */
+    out6[1] = (int32_t)(idx % pb->n_ap);      idx /= pb->n_ap;        /* ia  */
+    out6[0] = (int32_t)idx;                                           /* pix */
 }
 
 static inline int peak_bit(const uint32_t *peak, int32_t words_per_row, int32_t n_bins, int i, int64_t k)
@@ -205,10 +239,11 @@ void orc_stage1(const orc_problem *pb, int mode, const uint32_t *peak, int32_t w
     if (n_threads > 0) omp_set_num_threads(n_threads);
 #endif
     if (mode == ORC_DIRECT) {
-        const long n_outer = (long)pb->n_pix * pb->n_ap * pb->n_P * pb->n_tasc;
+        const long n_outer = (long)pb->n_pix * pb->n_ap * pb->n_P * pb->n_tasc * n_ecc_eff(pb);
 #pragma omp parallel for schedule(dynamic, 4)
         for (long o = 0; o < n_outer; ++o) {
             long r = o;
+            const int ie = (int)(r % n_ecc_eff(pb)); r /= n_ecc_eff(pb);
             const int it = (int)(r % pb->n_tasc); r /= pb->n_tasc;
             const int ip = (int)(r % pb->n_P);    r /= pb->n_P;
             const int ia = (int)(r % pb->n_ap);   r /= pb->n_ap;
@@ -217,13 +252,13 @@ void orc_stage1(const orc_problem *pb, int mode, const uint32_t *peak, int32_t w
                 int32_t n = 0;
                 double nw = 0.0;
                 for (int i = 0; i < N; ++i) {
-                    const int64_t k = orc_track_direct(pb, pix, ia, ip, it, j, i, NULL);
+                    const int64_t k = orc_track_direct(pb, pix, ia, ip, it, ie, j, i, NULL);
                     if (peak_bit(peak, words_per_row, pb->n_bins, i, k)) {
                         n += 1;
                         nw += w ? (double)w[i] : 1.0;
                     }
                 }
-                const uint64_t idx = tmpl_index(pb, pix, ia, ip, it, j);
+                const uint64_t idx = tmpl_index(pb, pix, ia, ip, it, ie, j);
                 if (count_out) count_out[idx] = n;
                 if (wcount_out) wcount_out[idx] = nw;
             }
@@ -247,10 +282,11 @@ void orc_stage1(const orc_problem *pb, int mode, const uint32_t *peak, int32_t w
             Ct[i] = cos(arg);
             St[i] = sin(arg);
         }
-        const long n_outer = (long)pb->n_pix * pb->n_ap * pb->n_tasc;
+        const long n_outer = (long)pb->n_pix * pb->n_ap * pb->n_tasc * n_ecc_eff(pb);
 #pragma omp parallel for schedule(dynamic, 4)
         for (long o = 0; o < n_outer; ++o) {
             long r = o;
+            const int ie = (int)(r % n_ecc_eff(pb)); r /= n_ecc_eff(pb);
             const int it = (int)(r % pb->n_tasc); r /= pb->n_tasc;
             const int ia = (int)(r % pb->n_ap);   r /= pb->n_ap;
             const int pix = (int)r;
@@ -264,13 +300,13 @@ void orc_stage1(const orc_problem *pb, int mode, const uint32_t *peak, int32_t w
                 int32_t n = 0;
                 double nw = 0.0;
                 for (int i = 0; i < N; ++i) {
-                    const int64_t k = canon_bin(pb, D[i], A, Ct[i], St[i], CA, SA, j, NULL);
+                    const int64_t k = canon_bin(pb, D[i], A, Ct[i], St[i], CA, SA, ecc_k(pb, ie), ecc_h(pb, ie), j, NULL);
                     if (peak_bit(peak, words_per_row, pb->n_bins, i, k)) {
                         n += 1;
                         nw += w ? (double)w[i] : 1.0;
                     }
                 }
-                const uint64_t idx = tmpl_index(pb, pix, ia, ip, it, j);
+                const uint64_t idx = tmpl_index(pb, pix, ia, ip, it, ie, j);
                 if (count_out) count_out[idx] = n;
                 if (wcount_out) wcount_out[idx] = nw;
             }
@@ -289,11 +325,12 @@ void orc_stage1(const orc_problem *pb, int mode, const uint32_t *peak, int32_t w
 void orc_compare_modes(const orc_problem *pb, double tol, int64_t *out)
 {
     int64_t n_cmp = 0, n_dis = 0, n_unfl = 0, n_flag = 0;
-    const long n_outer = (long)pb->n_pix * pb->n_ap * pb->n_P * pb->n_tasc;
+    const long n_outer = (long)pb->n_pix * pb->n_ap * pb->n_P * pb->n_tasc * n_ecc_eff(pb);
     const int64_t m = pb->k_band0 - pb->k_slab0;
 #pragma omp parallel for schedule(dynamic, 4) reduction(+ : n_cmp, n_dis, n_unfl, n_flag)
     for (long o = 0; o < n_outer; ++o) {
         long r = o;
+        const int ie = (int)(r % n_ecc_eff(pb)); r /= n_ecc_eff(pb);
         const int it = (int)(r % pb->n_tasc); r /= pb->n_tasc;
         const int ip = (int)(r % pb->n_P);    r /= pb->n_P;
         const int ia = (int)(r % pb->n_ap);   r /= pb->n_ap;
@@ -301,8 +338,8 @@ void orc_compare_modes(const orc_problem *pb, double tol, int64_t *out)
         for (int j = 0; j < pb->n_f0; ++j)
             for (int i = 0; i < pb->n_sft; ++i) {
                 double x, y;
-                const int64_t kd = orc_track_direct(pb, pix, ia, ip, it, j, i, &x);
-                const int64_t kc = orc_track_canonical(pb, pix, ia, ip, it, j, i, &y);
+                const int64_t kd = orc_track_direct(pb, pix, ia, ip, it, ie, j, i, &x);
+                const int64_t kc = orc_track_canonical(pb, pix, ia, ip, it, ie, j, i, &y);
                 const double xd = x + 0.5, xc = (double)(m + j) + y + 0.5;
                 const int flagged = fabs(xd - nearbyint(xd)) < tol || fabs(xc - nearbyint(xc)) < tol;
                 n_cmp += 1;
@@ -332,13 +369,14 @@ void orc_score(const orc_problem *pb, int mode, const uint64_t *idx, int64_t n_i
 #endif
 #pragma omp parallel for schedule(dynamic, 16)
     for (int64_t c = 0; c < n_idx; ++c) {
-        int32_t t5[5];
-        orc_decode_index(pb, idx[c], t5);
+        int32_t t6[6];
+        orc_decode_index(pb, idx[c], t6);
         int32_t n = 0;
         double nw = 0.0, pw = 0.0;
         for (int i = 0; i < pb->n_sft; ++i) {
-            const int64_t k = (mode == ORC_DIRECT) ? orc_track_direct(pb, t5[0], t5[1], t5[2], t5[3], t5[4], i, NULL)
-                                                   : orc_track_canonical(pb, t5[0], t5[1], t5[2], t5[3], t5[4], i, NULL);
+            const int64_t k = (mode == ORC_DIRECT)
+                                  ? orc_track_direct(pb, t6[0], t6[1], t6[2], t6[3], t6[4], t6[5], i, NULL)
+                                  : orc_track_canonical(pb, t6[0], t6[1], t6[2], t6[3], t6[4], t6[5], i, NULL);
             const double wi = w ? (double)w[i] : 1.0;
             if (peak && peak_bit(peak, words_per_row, pb->n_bins, i, k)) {
                 n += 1;

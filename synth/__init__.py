@@ -50,6 +50,8 @@ class Workload:
     tasc_frac: np.ndarray        # [n_t] f64 in [-0.5, 0.5): t_asc = t_search_mid + frac * P   (Eq. 35)
     topk: int
     rho_th: float = 1.6
+    ecosw: Optional[np.ndarray] = None   # [n_ecc] f64 e cos(omega), Eq. (14); None = circular orbits
+    esinw: Optional[np.ndarray] = None   # [n_ecc] f64 e sin(omega)
 
     @property
     def n_sft(self) -> int:
@@ -64,8 +66,12 @@ class Workload:
         return int(self.k_band0 - self.k_slab0)
 
     @property
+    def n_ecc(self) -> int:
+        return 0 if self.ecosw is None else int(len(self.ecosw))
+
+    @property
     def n_binary(self) -> int:
-        return len(self.ap) * len(self.P) * len(self.tasc_frac)
+        return len(self.ap) * len(self.P) * len(self.tasc_frac) * max(1, self.n_ecc)
 
     @property
     def n_templates(self) -> int:
@@ -386,6 +392,19 @@ def raw_sft_bins(seed: int, n_sft: int, n_raw: int, noise_sigma: float = 2.0) ->
     amp = np.exp(0.5 * noise_sigma * rng.standard_normal(n_sft))[:, None]
     slope = 1.0 + 0.3 * (np.arange(n_raw)[None, :] / max(n_raw, 1) - 0.5)
     return np.ascontiguousarray(x * amp * np.sqrt(slope), np.complex64)
+
+
+def eccentric(wl: Workload, e_max: float = 0.05, n_e: int = 2, n_omega: int = 3) -> Workload:
+    """The same workload with an eccentricity axis (Eq. 14, the ELL1 model for e << 1): pairs
+    (e cos omega, e sin omega) on n_e rings e = e_max m / n_e (m = 1..n_e) x n_omega arguments of periapsis, plus the
+    circular pair (0, 0) first.  Fig. 2 of the paper: most binary pulsars have e < 0.01; e_max = 0.05 keeps e << 1."""
+    ks, hs = [0.0], [0.0]
+    for m in range(1, n_e + 1):
+        for q in range(n_omega):
+            om = 2.0 * math.pi * (q + 0.25 * m) / n_omega
+            ks.append(e_max * m / n_e * math.cos(om))
+            hs.append(e_max * m / n_e * math.sin(om))
+    return dataclasses.replace(wl, name=wl.name + "-ecc", ecosw=np.asarray(ks, np.float64), esinw=np.asarray(hs, np.float64))
 
 
 def tie_workload() -> Workload:

@@ -522,3 +522,131 @@ def test_normalise_special_values():
     assert np.isnan(got[0, 0])                                               # centre bin is the NaN
     assert np.isclose(got[0, 1], np.float32(9.0) / (np.float32(16.0) / b3))
     assert np.isclose(got[0, 2], np.float32(16.0) / (np.float32(16.0) / b3))
+
+
+# ------------------------------------------------------------------------------------------------------------
+# Eccentric (ELL1) tracks: PAPER.md Eq. (14), derived from the timing model Eq. (11)-(13) L78-L91
+# ------------------------------------------------------------------------------------------------------------
+def test_eccentric_zero_pair_reproduces_circular_tracks_bit_for_bit():
+    wl = synth.config1(pixel="ecliptic")
+    we = synth.eccentric(wl)                                 # pair 0 is (0, 0)
+    assert we.n_ecc == 7 and we.n_templates == 7 * wl.n_templates and we.ecosw[0] == 0.0 and we.esinw[0] == 0.0
+    pk = oracle.peakgram(wl.rho)
+    for mode in (oracle.DIRECT, oracle.CANONICAL):
+        base_n, base_w = oracle.stage1(wl, pk, wl.w, mode=mode)
+        n, w = oracle.stage1(we, pk, wl.w, mode=mode)
+        shape = (1, 3, 3, 4, 7, 45)
+        assert np.array_equal(n.reshape(shape)[:, :, :, :, 0, :].ravel(), base_n)
+        assert np.array_equal(w.reshape(shape)[:, :, :, :, 0, :].ravel(), base_w)
+        assert not np.array_equal(n.reshape(shape)[:, :, :, :, 3, :].ravel(), base_n)     # e = 0.05 moves the tracks
+        for (ia, ip, it, j) in [(0, 0, 0, 0), (2, 1, 3, 44)]:
+            k0, a0 = oracle.track(wl, 0, ia, ip, it, j, mode=mode, with_aux=True)
+            k1, a1 = oracle.track(we, 0, ia, ip, it, j, mode=mode, with_aux=True, ie=0)
+            assert np.array_equal(k0, k1) and np.array_equal(a0, a1)
+    # index helpers with the extra axis
+    for idx in (0, 1, 44, 45, 7 * 45 - 1, 7 * 45, we.n_templates - 1, 12345):
+        pix, ia, ip, it, ie, j = oracle.decode_index(we, idx)
+        assert oracle.encode_index(we, pix, ia, ip, it, j, ie=ie) == idx
+
+
+def test_eccentric_track_bruteforce_eq14_50_digits():
+    """Eq. (14) as printed, in 50-digit arithmetic from the same FP64 inputs, against both oracle modes."""
+    mp.mp.dps = 50
+    we = synth.eccentric(synth.config1(pixel="pole"))
+    a, d = mp.mpf(we.alpha[0]), mp.mpf(we.delta[0])
+    nvec = (mp.cos(d) * mp.cos(a), mp.cos(d) * mp.sin(a), mp.sin(d))
+    D = [sum(mp.mpf(we.v_over_c[i, c]) * nvec[c] for c in range(3)) for i in range(we.n_sft)]
+    m = we.k_band0 - we.k_slab0
+    total = near = 0
+    for ip in range(len(we.P)):
+        P = mp.mpf(we.P[ip])
+        Om = 2 * mp.pi / P
+        for it in (0, 3):
+            tasc = mp.mpf(we.t_search_mid) + mp.mpf(we.tasc_frac[it]) * P
+            ph = [Om * (mp.mpf(we.t_mid[i]) - tasc) for i in range(we.n_sft)]
+            for ia in (0, 2):
+                ap = mp.mpf(we.ap[ia])
+                for ie in range(we.n_ecc):
+                    ecw, esw = mp.mpf(we.ecosw[ie]), mp.mpf(we.esinw[ie])
+                    g = [D[i] - ap * Om * mp.cos(ph[i]) - ap * Om * ecw * mp.cos(2 * ph[i]) + ap * Om * esw * mp.sin(2 * ph[i])
+                         for i in range(we.n_sft)]
+                    for j in (0, 13, 44):
+                        kd = oracle.track(we, 0, ia, ip, it, j, mode=oracle.DIRECT, ie=ie)
+                        kc = oracle.track(we, 0, ia, ip, it, j, mode=oracle.CANONICAL, ie=ie)
+                        u = mp.mpf(we.k_band0 + j)
+                        for i in range(we.n_sft):
+                            xh = m + j + u * g[i] + mp.mpf("0.5")
+                            total += 1
+                            if abs(xh - mp.nint(xh)) < mp.mpf("1e-9"):
+                                near += 1
+                                continue
+                            assert int(mp.floor(xh)) == kd[i] == kc[i], (ip, it, ia, ie, j, i)
+    assert total == 3 * 2 * 2 * 7 * 3 * 64 and near <= 2
+
+
+def test_eccentric_track_against_kepler_orbit_to_first_order_in_e():
+    """Independent of Eq. (14) as typed: the projected orbit of Eq. (9) (L68) with the eccentric anomaly from Kepler's
+    equation (7) and t_asc = t_p - omega / Omega (Eq. 10), differentiated numerically at 40 digits.  The ELL1 track
+    is its expansion to first order in e (L72, L80), so the two bin coordinates differ by at most ~ 2 e^2 a_p Omega u.
+    DESIGN.md R-24: expanding Eq. (9)-(10) gives R/c = a_p [sin psi + (e cos w / 2) sin 2 psi - (e sin w / 2) cos 2 psi];
+    Eq. (11)-(14) print the last term with the opposite sign.  The oracle follows Eq. (14) as printed, so its pair
+    (e cos w, e sin w) corresponds to the Kepler orbit with argument of periapsis -w: the test passes
+    esinw = -e sin(w_Kepler).  With esinw = +e sin(w_Kepler) the same comparison is off by O(e), which is asserted too."""
+    mp.mp.dps = 40
+    base = synth.config1(pixel="pole")
+    T = mp.mpf(base.t_sft)
+    for e, omega in [(0.01, 0.7), (0.03, 2.9), (0.002, 4.4)]:
+        we = dataclasses.replace(base, ecosw=np.array([e * math.cos(omega)]), esinw=np.array([-e * math.sin(omega)]))
+        wrong = dataclasses.replace(base, ecosw=np.array([e * math.cos(omega)]), esinw=np.array([e * math.sin(omega)]))
+        for (ia, ip, it, j) in [(2, 0, 1, 10), (0, 2, 3, 40)]:
+            P = mp.mpf(we.P[ip])
+            Om = 2 * mp.pi / P
+            ap, ee, om = mp.mpf(we.ap[ia]), mp.mpf(e), mp.mpf(omega)
+            tasc = mp.mpf(we.t_search_mid) + mp.mpf(we.tasc_frac[it]) * P
+            tp = tasc + om / Om                                                   # Eq. (10)
+            u = mp.mpf(we.k_band0 + j)
+
+            def roemer(t):                                                         # R(t)/c, Eq. (9) with Eq. (7)
+                M = Om * (t - tp)
+                E = mp.findroot(lambda x: x - ee * mp.sin(x) - M, M)
+                return ap * (mp.sin(om) * (mp.cos(E) - ee) + mp.cos(om) * mp.sin(E) * mp.sqrt(1 - ee * ee))
+
+            _, xd = oracle.track(we, 0, ia, ip, it, j, mode=oracle.DIRECT, with_aux=True, ie=0)
+            _, xw = oracle.track(wrong, 0, ia, ip, it, j, mode=oracle.DIRECT, with_aux=True, ie=0)
+            _, x0 = oracle.track(base, 0, ia, ip, it, j, mode=oracle.DIRECT, with_aux=True)
+            worst = worst_wrong = 0
+            for i in range(0, we.n_sft, 5):
+                t = mp.mpf(we.t_mid[i])
+                dR = mp.diff(roemer, t)                                            # f = f0 (1 + v.n/c - dR/dt), Eq. (13)
+                circ = -ap * Om * mp.cos(Om * (t - tasc))                          # the e = 0 term the circular track has
+                want_delta = u * (-dR - circ)                                      # bins the eccentricity moves the track by
+                got_delta = mp.mpf(xd[i]) - mp.mpf(x0[i])
+                worst = max(worst, abs(want_delta - got_delta))
+                worst_wrong = max(worst_wrong, abs(want_delta - (mp.mpf(xw[i]) - mp.mpf(x0[i]))))
+                assert abs(want_delta - got_delta) < 2.5 * ee * ee * ap * Om * u + mp.mpf("1e-7"), (e, omega, ia, ip, it, i)
+            assert worst_wrong > 0.5 * ee * abs(mp.sin(om)) * ap * Om * u          # the other sign is an O(e) error
+            # and the first-order terms are really there (a dropped or mis-signed term is O(e), not O(e^2))
+            assert max(abs(xd[i] - x0[i]) for i in range(we.n_sft)) > 0.5 * e * float(ap * Om * u) * 0.5
+
+
+def test_eccentric_modes_agree_and_symmetry():
+    wl = synth.eccentric(synth.noise_workload(seed=5, n_sft=300, n_f0=30, margin=44, f_band_start=150.0, n_pix_side=2,
+                                              ap=(10.0, 40.0), P_days=(15.0, 45.0), n_t=3), e_max=0.1)
+    res = oracle.compare_modes(wl, tol=1e-9)
+    assert res["compared"] == wl.n_accumulations and res["unflagged"] == 0
+    assert res["flagged"] < 40 + 4e-9 * res["compared"] * 5
+    # (a_p, t_asc, e cos w, e sin w) -> (-a_p, t_asc + P/2, -e cos w, -e sin w) is the same track (Eq. 14: phi -> phi - pi)
+    pk = oracle.peakgram(wl.rho)
+    base, _ = oracle.stage1(wl, pk, None, mode=oracle.DIRECT)
+    flipped = dataclasses.replace(wl, ap=-wl.ap, tasc_frac=wl.tasc_frac + 0.5, ecosw=-wl.ecosw, esinw=-wl.esinw)
+    got, _ = oracle.stage1(flipped, pk, None, mode=oracle.DIRECT)
+    assert np.array_equal(base, got)
+    # hoisted CANONICAL loop == per-accumulation canonical track, eccentric templates included
+    bits = np.unpackbits(pk.view(np.uint8), axis=1, bitorder="little")[:, :wl.n_bins]
+    cnt, _ = oracle.stage1(wl, pk, None, mode=oracle.CANONICAL)
+    rows = np.arange(wl.n_sft)
+    for idx in range(3, wl.n_templates, 97):
+        pix, ia, ip, it, ie, j = oracle.decode_index(wl, idx)
+        k = oracle.track(wl, pix, ia, ip, it, j, mode=oracle.CANONICAL, ie=ie)
+        inside = (k >= 0) & (k < wl.n_bins)
+        assert cnt[idx] == bits[rows[inside], k[inside]].sum()
