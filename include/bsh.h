@@ -19,7 +19,8 @@
  *   - All device work is enqueued on the CUDA stream given to bsh_create().  Functions documented "asynchronous"
  *     return before the work completes; the caller synchronises that stream before reading results.
  *   - There is no CPU fallback: without a CUDA device bsh_create() fails with BSH_ECUDA.
- *   - Template linear index (R-11): ((((pix * n_ap + ia) * n_P + ip) * n_tasc + it) * n_f0 + j, f0 fastest.
+ *   - Template linear index (R-11): ((((pix * n_ap + ia) * n_P + ip) * n_tasc + it) * n_f0 + j, f0 fastest; with an
+ *     eccentricity axis: (((((pix * n_ap + ia) * n_P + ip) * n_tasc + it) * n_ecc + ie) * n_f0 + j.
  *   - Ordering everywhere: (statistic descending, template index ascending).
  */
 #ifndef BSH_H_
@@ -79,6 +80,10 @@ typedef struct {
     int32_t n_ap;   const double *h_ap;               /* [n_ap]  projected semi-major axis, light-seconds (L70)    */
     int32_t n_P;    const double *h_P;                /* [n_P]   orbital period, seconds                           */
     int32_t n_tasc; const double *h_tasc_frac;        /* [n_tasc] t_asc = t_search_mid + frac * P (Eq. 35, R-13)   */
+    /* Eccentric orbits (ELL1 model, Eq. 14): n_ecc pairs (e cos omega, e sin omega); the track is
+     * f(t) = f0 [1 + v.n/c - a_p Omega (cos phi + ecosw cos 2 phi - esinw sin 2 phi)], phi = Omega (t - t_asc), as Eq. (14)
+     * prints it (readings R-23, R-24).  n_ecc = 0 (pointers ignored): circular orbits, Eq. (15).                          */
+    int32_t n_ecc;  const double *h_ecosw, *h_esinw;  /* [n_ecc]                                                     */
 } bsh_grid;
 
 /* Toplist / candidate record (24 bytes). */
@@ -197,10 +202,14 @@ int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, c
 int bsh_search_patch_host(bsh_ctx *ctx, const float *h_rho, const float *h_w, float rho_th, const bsh_sfts *sfts,
                           const bsh_grid *grid, int32_t mode, int32_t topk, bsh_cand *h_top, int32_t *h_n_top);
 
-/* Template index helpers (R-11).  Pure host functions. */
+/* Template index helpers (R-11).  Pure host functions.  The first pair is for circular grids (n_ecc = 0; on an eccentric
+ * grid it addresses pair ie = 0 / drops ie); the _ecc pair carries the eccentricity index. */
 uint64_t bsh_template_index(const bsh_grid *grid, int32_t pix, int32_t ia, int32_t ip, int32_t it, int32_t j);
 void     bsh_template_decode(const bsh_grid *grid, uint64_t index, int32_t *pix, int32_t *ia, int32_t *ip,
                              int32_t *it, int32_t *j);
+uint64_t bsh_template_index_ecc(const bsh_grid *grid, int32_t pix, int32_t ia, int32_t ip, int32_t it, int32_t ie, int32_t j);
+void     bsh_template_decode_ecc(const bsh_grid *grid, uint64_t index, int32_t *pix, int32_t *ia, int32_t *ip,
+                                 int32_t *it, int32_t *ie, int32_t *j);
 
 #ifdef __cplusplus
 }

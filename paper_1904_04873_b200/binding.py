@@ -16,7 +16,7 @@ BSH_FAMILY_AUTO, BSH_FAMILY_PIXEL_LANE, BSH_FAMILY_TEMPLATE_LANE, BSH_FAMILY_WIN
 EXPORTS = ["bsh_version", "bsh_create", "bsh_destroy", "bsh_last_error", "bsh_get_stats", "bsh_set_option",
            "bsh_measure_peaks", "bsh_build_peakgram", "bsh_normalise_peakgram", "bsh_median_bias",
            "bsh_stage1_hough", "bsh_stage1_launch", "bsh_stage1_collect", "bsh_stage2_power", "bsh_search_patch_host",
-           "bsh_template_index", "bsh_template_decode"]
+           "bsh_template_index", "bsh_template_decode", "bsh_template_index_ecc", "bsh_template_decode_ecc"]
 
 # numpy view of bsh_cand (24 bytes)
 CAND_DTYPE = np.dtype([("index", "<u8"), ("count", "<i4"), ("wcount", "<f4"), ("power", "<f4"), ("flags", "<u4")])
@@ -34,7 +34,8 @@ class _Sfts(C.Structure):
 class _Grid(C.Structure):
     _fields_ = [("n_pix", C.c_int32), ("h_alpha", C.c_void_p), ("h_delta", C.c_void_p), ("k_band0", C.c_int64),
                 ("n_f0", C.c_int32), ("n_ap", C.c_int32), ("h_ap", C.c_void_p), ("n_P", C.c_int32), ("h_P", C.c_void_p),
-                ("n_tasc", C.c_int32), ("h_tasc_frac", C.c_void_p)]
+                ("n_tasc", C.c_int32), ("h_tasc_frac", C.c_void_p),
+                ("n_ecc", C.c_int32), ("h_ecosw", C.c_void_p), ("h_esinw", C.c_void_p)]
 
 
 class Stats(C.Structure):
@@ -71,6 +72,8 @@ def library():
         lib.bsh_last_error.restype = C.c_char_p
         lib.bsh_template_index.restype = C.c_uint64
         lib.bsh_template_decode.restype = None
+        lib.bsh_template_index_ecc.restype = C.c_uint64
+        lib.bsh_template_decode_ecc.restype = None
         lib.bsh_median_bias.restype = C.c_double
         for name in EXPORTS:
             getattr(lib, name)                       # fail loudly on a missing symbol
@@ -85,6 +88,10 @@ class _Problem:
         f64 = lambda a: np.ascontiguousarray(a, np.float64)
         self.a = dict(t_mid=f64(wl.t_mid), v=f64(wl.v_over_c), alpha=f64(wl.alpha), delta=f64(wl.delta), ap=f64(wl.ap),
                       P=f64(wl.P), tf=f64(wl.tasc_frac))
+        ecw = getattr(wl, "ecosw", None)
+        n_ecc = 0 if ecw is None else len(ecw)
+        if n_ecc:
+            self.a.update(ecw=f64(ecw), esw=f64(wl.esinw))
         a = self.a
         self.sfts = _Sfts(n_sft=a["t_mid"].shape[0], t_sft=float(wl.t_sft), h_t_mid=a["t_mid"].ctypes.data,
                           h_v_over_c=a["v"].ctypes.data, d_w=(d_w.data_ptr() if d_w is not None else None),
@@ -92,7 +99,8 @@ class _Problem:
         self.grid = _Grid(n_pix=a["alpha"].shape[0], h_alpha=a["alpha"].ctypes.data, h_delta=a["delta"].ctypes.data,
                           k_band0=int(wl.k_band0), n_f0=int(wl.n_f0), n_ap=a["ap"].shape[0], h_ap=a["ap"].ctypes.data,
                           n_P=a["P"].shape[0], h_P=a["P"].ctypes.data, n_tasc=a["tf"].shape[0],
-                          h_tasc_frac=a["tf"].ctypes.data)
+                          h_tasc_frac=a["tf"].ctypes.data, n_ecc=n_ecc, h_ecosw=a["ecw"].ctypes.data if n_ecc else None,
+                          h_esinw=a["esw"].ctypes.data if n_ecc else None)
         self.d_w = d_w
 
 
@@ -102,6 +110,16 @@ def median_bias(window: int = 101) -> float:
 
 def template_index(wl, pix, ia, ip, it, j) -> int:
     return int(library().bsh_template_index(C.byref(_Problem(wl).grid), pix, ia, ip, it, j))
+
+
+def template_index_ecc(wl, pix, ia, ip, it, ie, j) -> int:
+    return int(library().bsh_template_index_ecc(C.byref(_Problem(wl).grid), pix, ia, ip, it, ie, j))
+
+
+def template_decode_ecc(wl, index):
+    out = [C.c_int32() for _ in range(6)]
+    library().bsh_template_decode_ecc(C.byref(_Problem(wl).grid), C.c_uint64(int(index)), *[C.byref(o) for o in out])
+    return tuple(o.value for o in out)
 
 
 def template_decode(wl, index):

@@ -36,10 +36,10 @@ struct DevBuf {
 struct TableCache {                   // cos/sin tables of one (SFT set, binary grid); content-addressed
     bool valid = false;
     uint64_t stamp = 0;
-    std::vector<double> t_mid, v, P, tasc, ap;
+    std::vector<double> t_mid, v, P, tasc, ap, ecw, esw;
     double t_sft = 0, t_search_mid = 0;
-    int n_sft = 0, n_pad = 0, n_P = 0, n_tasc = 0, n_ap = 0;
-    DevBuf d_v, d_cs, d_casa, d_A;
+    int n_sft = 0, n_pad = 0, n_P = 0, n_tasc = 0, n_ap = 0, n_ecc = 0;
+    DevBuf d_v, d_cs, d_casa, d_A, d_ke;
 };
 
 struct Pending {                      // state between bsh_stage1_launch and bsh_stage1_collect
@@ -157,6 +157,25 @@ static_assert(kHostChunk == kChunk, "SFT padding granularity");
 // Host tables (R-5).  The only transcendental evaluations of the whole path: libm cos/sin of Omega_p t_i and
 // Omega_p t_asc, and of the pixel angles.  Cached by content: a sweep over sky patches reuses them.
 // ---------------------------------------------------------------------------------------------------------------------
+inline int n_ecc_of(const bsh_grid *g) { return g->n_ecc > 0 ? g->n_ecc : 0; }
+inline int n_tq_of(const bsh_grid *g) { return g->n_tasc * (g->n_ecc > 0 ? g->n_ecc : 1); }   // combined (t_asc, eccentricity) axis
+
+// the grid as the kernels see it: the eccentricity axis folded into the t_asc axis (bsh_host.hpp, build_binary_tables)
+inline bsh_grid kernel_grid(const bsh_grid *g)
+{
+    bsh_grid k = *g;
+    k.n_tasc = n_tq_of(g);
+    k.n_ecc = 0;
+    return k;
+}
+
+double ecc_max_of(const bsh_grid *g)
+{
+    double m = 0.0;
+    for (int e = 0; e < n_ecc_of(g); ++e) m = std::max(m, fabs(g->h_ecosw[e]) + fabs(g->h_esinw[e]));
+    return m;
+}
+
 int validate(bsh_ctx *ctx, const bsh_sfts *s, const bsh_grid *g)
 {
     if (!s || !g) return fail(ctx, BSH_EINVAL, "null sfts/grid");
@@ -170,6 +189,10 @@ int validate(bsh_ctx *ctx, const bsh_sfts *s, const bsh_grid *g)
         return fail(ctx, BSH_EINVAL, "band offset out of range");
     for (int p = 0; p < g->n_P; ++p)
         if (!(g->h_P[p] > 0)) return fail(ctx, BSH_EINVAL, "P[%d] <= 0", p);
+    if (g->n_ecc < 0 || (g->n_ecc > 0 && (!g->h_ecosw || !g->h_esinw))) return fail(ctx, BSH_EINVAL, "bad eccentricity axis");
+    for (int e = 0; e < n_ecc_of(g); ++e)
+        if (!(fabs(g->h_ecosw[e]) + fabs(g->h_esinw[e]) < 1.0)) return fail(ctx, BSH_EINVAL, "eccentricity pair %d out of range", e);
+    if ((int64_t)g->n_tasc * std::max(1, g->n_ecc) > (1 << 24)) return fail(ctx, BSH_EINVAL, "t_asc x eccentricity axis too long");
     return BSH_OK;
 }
 
@@ -179,6 +202,8 @@ int get_tables(bsh_ctx *ctx, const bsh_sfts *s, const bsh_grid *g, int *slot_out
     for (int k = 0; k < 2; ++k) {
         TableCache &c = ctx->cache[k];
         if (c.valid && c.n_sft == N && c.n_P == g->n_P && c.n_tasc == g->n_tasc && c.n_ap == g->n_ap &&
+            c.n_ecc == n_ecc_of(g) && (c.n_ecc == 0 || (!memcmp(c.ecw.data(), g->h_ecosw, sizeof(double) * c.n_ecc) &&
+                                                         !memcmp(c.esw.data(), g->h_esinw, sizeof(double) * c.n_ecc))) &&
             c.t_sft == s->t_sft && c.t_search_mid == s->t_search_mid &&
             !memcmp(c.t_mid.data(), s->h_t_mid, sizeof(double) * N) &&
             !memcmp(c.v.data(), s->h_v_over_c, sizeof(double) * 3 * N) &&
@@ -204,11 +229,15 @@ int get_tables(bsh_ctx *ctx, const bsh_sfts *s, const bsh_grid *g, int *slot_out
     c.ap.assign(g->h_ap, g->h_ap + g->n_ap);
     c.t_sft = s->t_sft;
     c.t_search_mid = s->t_search_mid;
-    c.n_sft = N; c.n_pad = n_pad; c.n_P = g->n_P; c.n_tasc = g->n_tasc; c.n_ap = g->n_ap;
+    c.n_sft = N; c.n_pad = n_pad; c.n_P = g->n_P; c.n_tasc = g->n_tasc; c.n_ap = g->n_ap; c.n_ecc = n_ecc_of(g);
+    c.ecw.assign(g->h_ecosw, g->h_ecosw + c.n_ecc);
+    c.esw.assign(g->h_esinw, g->h_esinw + c.n_ecc);
 
-    std::vector<double> cs, casa, A;
+    std::vector<double> cs, casa, A, ke;
     build_binary_tables(N, n_pad, s->h_t_mid, s->t_search_mid, g->n_P, g->h_P, g->n_tasc, g->h_tasc_frac, g->n_ap, g->h_ap, cs,
-                        casa, A);
+                        casa, A, c.n_ecc, g->h_ecosw, g->h_esinw, &ke);
+    TRY(ensure(ctx, c.d_ke, sizeof(double) * ke.size()));
+    CK(cudaMemcpyAsync(c.d_ke.p, ke.data(), sizeof(double) * ke.size(), cudaMemcpyHostToDevice, ctx->stream));
     TRY(ensure(ctx, c.d_v, sizeof(double) * 3 * (size_t)N));
     TRY(ensure(ctx, c.d_cs, sizeof(double) * cs.size()));
     TRY(ensure(ctx, c.d_casa, sizeof(double) * casa.size()));
@@ -250,6 +279,7 @@ TrackTables make_track_tables(const TableCache &c, const bsh_sfts *s, const bsh_
     t.dtab = dtab;
     t.A = (const double *)c.d_A.p;
     t.casa = (const double2 *)c.d_casa.p;
+    t.ke = c.n_ecc > 0 ? (const double2 *)c.d_ke.p : nullptr;
     t.n_pad = c.n_pad;
     t.R = R;
     t.n_pix = g->n_pix; t.n_ap = g->n_ap; t.n_P = g->n_P; t.n_tasc = g->n_tasc; t.n_f0 = g->n_f0;
@@ -400,6 +430,7 @@ int run_pass(bsh_ctx *ctx)
             p.w_pad = (const float *)ctx->w_pad.p;
             p.A = (const double *)c.d_A.p;
             p.casa = (const double2 *)c.d_casa.p;
+            p.ke = c.n_ecc > 0 ? (const double2 *)c.d_ke.p : nullptr;
             p.n_pad = pd.n_pad; p.n_pos = pd.n_pos; p.n_chunks = pd.n_pad / kStageSfts; p.n_stages = pd.wpix_stages;
             p.n_pix = pd.n_pix; p.n_ap = pd.n_ap; p.n_P = pd.n_P; p.n_tasc = pd.n_tasc; p.n_f0 = pd.n_f0;
             p.j0 = j0; p.n_fj = std::min(tile_bins, pd.n_f0 - j0);
@@ -431,6 +462,7 @@ int run_pass(bsh_ctx *ctx)
             p.zero = 0u;
             p.A = (const double *)c.d_A.p;
             p.casa = (const double2 *)c.d_casa.p;
+            p.ke = c.n_ecc > 0 ? (const double2 *)c.d_ke.p : nullptr;
             p.n_pad = pd.n_pad; p.n_pos = pd.n_pos; p.n_chunks = pd.n_pad / kStageSfts; p.n_stages = pd.pix_stages;
             p.n_pix = pd.n_pix; p.n_ap = pd.n_ap; p.n_P = pd.n_P; p.n_tasc = pd.n_tasc; p.n_f0 = pd.n_f0;
             p.j0 = j0; p.n_fj = std::min(tile_bins, pd.n_f0 - j0);
@@ -460,6 +492,7 @@ int run_pass(bsh_ctx *ctx)
             p.w_pad = (const float *)ctx->w_pad.p;
             p.A = (const double *)c.d_A.p;
             p.casa = (const double2 *)c.d_casa.p;
+            p.ke = c.n_ecc > 0 ? (const double2 *)c.d_ke.p : nullptr;
             p.n_pad = pd.n_pad; p.n_pos = pd.n_pos; p.n_chunks = pd.n_pad / kStageSfts; p.n_stages = pd.n_stages;
             p.n_pix = pd.n_pix; p.n_ap = pd.n_ap; p.n_P = pd.n_P; p.n_tasc = pd.n_tasc; p.n_f0 = pd.n_f0;
             p.j0 = j0; p.n_fj = std::min(tile_bins, pd.n_f0 - j0);
@@ -489,6 +522,7 @@ int run_pass(bsh_ctx *ctx)
             p.w_pad = (const float *)ctx->w_pad.p;
             p.A = (const double *)c.d_A.p;
             p.casa = (const double2 *)c.d_casa.p;
+            p.ke = c.n_ecc > 0 ? (const double2 *)c.d_ke.p : nullptr;
             p.n_pad = pd.n_pad; p.n_entries = pd.n_entries; p.n_chunks = pd.n_pad / kChunk;
             p.n_pix = pd.n_pix; p.n_ap = pd.n_ap; p.n_P = pd.n_P; p.n_tasc = pd.n_tasc; p.n_f0 = pd.n_f0;
             p.j0 = j0; p.n_fj = std::min(tile_bins, pd.n_f0 - j0);
@@ -606,7 +640,7 @@ int bsh_destroy(bsh_ctx *ctx)
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto &c : ctx->cache) {
-        DevBuf *cb[] = {&c.d_v, &c.d_cs, &c.d_casa, &c.d_A};
+        DevBuf *cb[] = {&c.d_v, &c.d_cs, &c.d_casa, &c.d_A, &c.d_ke};
         for (DevBuf *b : cb)
             if (b->p) cudaFree(b->p);
     }
@@ -766,8 +800,10 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     pd.mode = mode; pd.topk = topk; pd.d_counts_full = d_counts_full; pd.d_peak = d_peak;
     pd.words_per_row = words_per_row; pd.d_w = sfts->d_w;
     pd.n_sft = sfts->n_sft; pd.n_bins = sfts->n_bins; pd.n_pix = grid->n_pix; pd.n_ap = grid->n_ap; pd.n_P = grid->n_P;
-    pd.n_tasc = grid->n_tasc; pd.n_f0 = grid->n_f0; pd.k_band0 = grid->k_band0; pd.k_slab0 = sfts->k_slab0;
-    pd.n_templates = (uint64_t)grid->n_pix * grid->n_ap * grid->n_P * grid->n_tasc * (uint64_t)grid->n_f0;
+    const bsh_grid kg = kernel_grid(grid);             // eccentricity axis folded into the t_asc axis
+    const double ecc_max = ecc_max_of(grid);
+    pd.n_tasc = kg.n_tasc; pd.n_f0 = grid->n_f0; pd.k_band0 = grid->k_band0; pd.k_slab0 = sfts->k_slab0;
+    pd.n_templates = (uint64_t)grid->n_pix * grid->n_ap * grid->n_P * kg.n_tasc * (uint64_t)grid->n_f0;
     const bool weighted = (mode & BSH_WEIGHTED) != 0;
 
     TRY(get_tables(ctx, sfts, grid, &pd.cache_slot));
@@ -798,7 +834,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         const int nbytes = tile <= 48 ? 8 : 15, nw = nbytes == 8 ? 2 : 3;
         const TableGeometry tgw = table_geometry(sfts->n_sft, sfts->h_v_over_c, grid->n_P, grid->h_P, grid->n_ap, grid->h_ap,
                                                  grid->k_band0, sfts->k_slab0, grid->n_f0, sfts->n_bins, nw,
-                                                 ctx->opt_force_clamp != 0);
+                                                 ctx->opt_force_clamp != 0, ecc_max);
         const PosGeometry pgw = pos_geometry(tgw, sfts->n_bins, grid->n_f0, nw, tile);
         const WpixStage ws(pgw.n_pos, wpix_entry_bytes(nbytes));
         const int stages = std::min(kMaxStages, (220 * 1024 - kWpixHeader) / ws.stride);     // one block per SM
@@ -814,10 +850,10 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     if (sfts->n_sft >= (1 << 16)) return fail(ctx, BSH_EINVAL, "n_sft >= 65536 not supported");
     const TableGeometry tg = table_geometry(sfts->n_sft, sfts->h_v_over_c, grid->n_P, grid->h_P, grid->n_ap, grid->h_ap,
                                             grid->k_band0, sfts->k_slab0, grid->n_f0, sfts->n_bins, pd.NW,
-                                            ctx->opt_force_clamp != 0);
+                                            ctx->opt_force_clamp != 0, ecc_max);
     pd.clamp = tg.clamp; pd.off_table = tg.off_table; pd.s_max = tg.s_max; pd.n_entries = tg.n_entries;
     pd.s_zero = tg.s_zero;
-    const int n_aq = grid->n_ap * grid->n_tasc;
+    const int n_aq = grid->n_ap * kg.n_tasc;
     pd.tpb = pick_threads_per_block(n_aq);
     pd.n_aq_tiles = (n_aq + pd.tpb - 1) / pd.tpb;
     pd.list_cap = 48;
@@ -1050,7 +1086,8 @@ int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, c
     const TableCache &c = ctx->cache[slot];
     CK(cudaEventRecord(ctx->ev[6], ctx->stream));
     TRY(build_dtable(ctx, grid, c, 1, ctx->nvec2, ctx->dtab2));
-    const TrackTables t = make_track_tables(c, sfts, grid, (const double *)ctx->dtab2.p, 1);
+    const bsh_grid kg = kernel_grid(grid);
+    const TrackTables t = make_track_tables(c, sfts, &kg, (const double *)ctx->dtab2.p, 1);
     stage2_kernel<<<(unsigned)n_cands, kCandThreads, 0, ctx->stream>>>(t, d_rho, rho_row_stride,
                                                                                           sfts->d_w, d_cands, n_cands);
     count_launch(ctx);
@@ -1101,13 +1138,34 @@ int bsh_search_patch_host(bsh_ctx *ctx, const float *h_rho, const float *h_w, fl
     return BSH_OK;
 }
 
+uint64_t bsh_template_index_ecc(const bsh_grid *g, int32_t pix, int32_t ia, int32_t ip, int32_t it, int32_t ie, int32_t j)
+{
+    const uint64_t ne = g->n_ecc > 0 ? (uint64_t)g->n_ecc : 1u;
+    return (((((uint64_t)pix * g->n_ap + ia) * g->n_P + ip) * g->n_tasc + it) * ne + ie) * (uint64_t)g->n_f0 + j;
+}
+
 uint64_t bsh_template_index(const bsh_grid *g, int32_t pix, int32_t ia, int32_t ip, int32_t it, int32_t j)
 {
-    return ((((uint64_t)pix * g->n_ap + ia) * g->n_P + ip) * g->n_tasc + it) * (uint64_t)g->n_f0 + j;
+    return bsh_template_index_ecc(g, pix, ia, ip, it, 0, j);
+}
+
+void bsh_template_decode_ecc(const bsh_grid *g, uint64_t idx, int32_t *pix, int32_t *ia, int32_t *ip, int32_t *it, int32_t *ie,
+                             int32_t *j)
+{
+    const uint64_t ne = g->n_ecc > 0 ? (uint64_t)g->n_ecc : 1u;
+    const int32_t jj = (int32_t)(idx % (uint64_t)g->n_f0);   idx /= (uint64_t)g->n_f0;
+    const int32_t ee = (int32_t)(idx % ne);                  idx /= ne;
+    if (ie) *ie = ee;
+    bsh_grid k = *g;
+    k.n_ecc = 0;
+    k.n_f0 = 1;
+    bsh_template_decode(&k, idx, pix, ia, ip, it, nullptr);
+    if (j) *j = jj;
 }
 
 void bsh_template_decode(const bsh_grid *g, uint64_t idx, int32_t *pix, int32_t *ia, int32_t *ip, int32_t *it, int32_t *j)
 {
+    if (g->n_ecc > 0) { bsh_template_decode_ecc(g, idx, pix, ia, ip, it, nullptr, j); return; }
     const int32_t jj = (int32_t)(idx % (uint64_t)g->n_f0);   idx /= (uint64_t)g->n_f0;
     const int32_t tt = (int32_t)(idx % (uint64_t)g->n_tasc); idx /= (uint64_t)g->n_tasc;
     const int32_t pp = (int32_t)(idx % (uint64_t)g->n_P);    idx /= (uint64_t)g->n_P;

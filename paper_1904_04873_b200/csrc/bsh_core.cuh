@@ -106,6 +106,7 @@ struct TrackConst {
     double u0, uL;      // k_band0 + j0  and  k_band0 + j0 + n_fj - 1
     double A;           // fl(a_p Omega)
     double CA, SA;      // cos / sin (Omega t_asc)  (host libm table values)
+    double kap, eta;    // e cos(omega), e sin(omega) of the ELL1 track, Eq. (14) (0, 0: circular orbit, Eq. 15)
     double magic;       // kMagic + off
     int32_t off;        // m + j0 + table offset: s = off + r is the bit position of tile bin 0 in table coordinates
     int32_t s_max;      // clamp range [0, s_max] of s (table coordinates); only used by CLAMP variants
@@ -215,9 +216,25 @@ BSH_HD Win<NW> track_window_deferred(const TrackConst &tc, const uint4 *row_entr
     return load_window<NW>(row_entries, s);
 }
 
-BSH_HD double binary_term(const TrackConst &tc, double C, double S)   // B = fl(A fl(fl(C CA) + fl(S SA)))
+// The bracket of the binary term of Eq. (14) (L95-L98):  cos phi + kap cos 2 phi - eta sin 2 phi,  phi = Omega (t - t_asc),
+// from the table values (C, S) = (cos, sin)(Omega t), (CA, SA) = (cos, sin)(Omega t_asc) with rounded +, -, * only
+// (R-23):  cos phi = fl(fl(C CA) + fl(S SA)),  sin phi = fl(fl(S CA) - fl(C SA)),
+// cos 2 phi = fl(fl(cos^2 phi) - fl(sin^2 phi)),  sin 2 phi = fl(fl(2 sin phi) cos phi),
+// E = fl(fl(kap cos 2 phi) - fl(eta sin 2 phi)),  bracket = fl(cos phi + E).  kap = eta = 0 is Eq. (15): cos phi.
+BSH_HD double orbit_bracket(double C, double S, double CA, double SA, double kap, double eta)
 {
-    return dmul(tc.A, dadd(dmul(C, tc.CA), dmul(S, tc.SA)));
+    const double cphi = dadd(dmul(C, CA), dmul(S, SA));
+    if (kap == 0.0 && eta == 0.0) return cphi;
+    const double sphi = dsub(dmul(S, CA), dmul(C, SA));
+    const double cos2 = dsub(dmul(cphi, cphi), dmul(sphi, sphi));
+    const double sin2 = dmul(dmul(2.0, sphi), cphi);
+    const double E = dsub(dmul(kap, cos2), dmul(eta, sin2));
+    return dadd(cphi, E);
+}
+
+BSH_HD double binary_term(const TrackConst &tc, double C, double S)   // B = fl(A bracket)
+{
+    return dmul(tc.A, orbit_bracket(C, S, tc.CA, tc.SA, tc.kap, tc.eta));
 }
 
 // ---------------------------------------------------------------------------------------------------------------------

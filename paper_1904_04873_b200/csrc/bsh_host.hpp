@@ -16,13 +16,27 @@ inline int pad_sfts(int n) { return (n + kHostChunk - 1) / kHostChunk * kHostChu
 
 // cs[p][i] = (cos, sin)(Omega_p t_i) for i < n_sft, (0, 0) for the padding SFTs;  casa[p][q] = (cos, sin)(Omega_p t_asc),
 // t_asc = t_search_mid + frac_q P_p (Eq. 35);  A[a][p] = a_p Omega_p;  Omega_p = (2 pi) / P_p (L61).
+// Eccentric grids (Eq. 14; n_ecc > 0): the kernels see ONE combined axis tq = q n_ecc + e of n_tasc n_ecc entries -- casa is
+// replicated over e, and ke[tq] = (e cos omega, e sin omega)_e -- so the template index keeps its R-11 form with the
+// eccentricity pair between t_asc and f0.
 inline void build_binary_tables(int n_sft, int n_pad, const double *t_mid, double t_search_mid, int n_P, const double *P,
                                 int n_tasc, const double *tasc_frac, int n_ap, const double *ap, std::vector<double> &cs,
-                                std::vector<double> &casa, std::vector<double> &A)
+                                std::vector<double> &casa, std::vector<double> &A, int n_ecc = 0,
+                                const double *ecosw = nullptr, const double *esinw = nullptr,
+                                std::vector<double> *ke = nullptr)
 {
+    const int ne = n_ecc > 0 ? n_ecc : 1;
     cs.assign((size_t)n_P * n_pad * 2, 0.0);
-    casa.assign((size_t)n_P * n_tasc * 2, 0.0);
+    casa.assign((size_t)n_P * n_tasc * ne * 2, 0.0);
     A.assign((size_t)n_ap * n_P, 0.0);
+    if (ke) {
+        ke->assign((size_t)n_tasc * ne * 2, 0.0);
+        for (int q = 0; q < n_tasc; ++q)
+            for (int e = 0; e < n_ecc; ++e) {
+                (*ke)[((size_t)q * ne + e) * 2 + 0] = ecosw[e];
+                (*ke)[((size_t)q * ne + e) * 2 + 1] = esinw[e];
+            }
+    }
     const double two_pi = 2.0 * M_PI;
     for (int p = 0; p < n_P; ++p) {
         const double Pp = P[p];
@@ -36,8 +50,11 @@ inline void build_binary_tables(int n_sft, int n_pad, const double *t_mid, doubl
             const double fp = tasc_frac[q] * Pp;
             const double ta = t_search_mid + fp;
             const double arg = Om * ta;
-            casa[((size_t)p * n_tasc + q) * 2 + 0] = cos(arg);
-            casa[((size_t)p * n_tasc + q) * 2 + 1] = sin(arg);
+            const double ca = cos(arg), sa = sin(arg);
+            for (int e = 0; e < ne; ++e) {
+                casa[(((size_t)p * n_tasc + q) * ne + e) * 2 + 0] = ca;
+                casa[(((size_t)p * n_tasc + q) * ne + e) * 2 + 1] = sa;
+            }
         }
         for (int a = 0; a < n_ap; ++a) A[(size_t)a * n_P + p] = ap[a] * Om;
     }
@@ -67,7 +84,8 @@ struct TableGeometry {
 };
 
 inline TableGeometry table_geometry(int n_sft, const double *v_over_c, int n_P, const double *P, int n_ap, const double *ap,
-                                    int64_t k_band0, int64_t k_slab0, int n_f0, int n_bins, int NW, bool force_clamp)
+                                    int64_t k_band0, int64_t k_slab0, int n_f0, int n_bins, int NW, bool force_clamp,
+                                    double ecc_max = 0.0 /* max |e cos w| + |e sin w| of the grid (Eq. 14) */)
 {
     double vmax = 0;
     for (int i = 0; i < n_sft; ++i) {
@@ -77,7 +95,7 @@ inline TableGeometry table_geometry(int n_sft, const double *v_over_c, int n_P, 
     double pmin = P[0], apmax = 0;
     for (int p = 0; p < n_P; ++p) pmin = std::min(pmin, P[p]);
     for (int a = 0; a < n_ap; ++a) apmax = std::max(apmax, fabs(ap[a]));
-    const double amax = apmax * 2.0 * M_PI / pmin;
+    const double amax = apmax * 2.0 * M_PI / pmin * (1.0 + ecc_max);   // |cos phi + k cos 2 phi - h sin 2 phi| <= 1 + |k| + |h|
     // |r| <= |y| + 1/2 rounded, |y| <= u_max (|v|/c + a_p Omega); generous relative slack for the rounded operations
     const double rmax = floor((double)(k_band0 + n_f0) * (vmax * 1.000001 + amax * 1.000001) + 0.5) + 1.0;
     const int64_t m = k_band0 - k_slab0;

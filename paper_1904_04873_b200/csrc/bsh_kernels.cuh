@@ -212,6 +212,7 @@ struct Stage1Params {
     const float *w_pad;         // [n_pad]
     const double *A;            // [n_ap][n_P]   fl(a_p Omega_p)
     const double2 *casa;        // [n_P][n_tasc] (cos, sin)(Omega_p t_asc)
+    const double2 *ke;          // [n_tasc] (e cos omega, e sin omega) of the combined (t_asc, eccentricity) axis, or NULL
     int n_pad, n_entries, n_chunks;
     int n_pix, n_ap, n_P, n_tasc, n_f0;
     int j0, n_fj;               // f0 tile
@@ -256,6 +257,9 @@ __device__ __forceinline__ TrackConst make_track_const(const Stage1Params &p, co
     const double2 q = p.casa[c.ip * p.n_tasc + c.it];
     tc.CA = q.x;
     tc.SA = q.y;
+    const double2 ke = p.ke ? p.ke[c.it] : make_double2(0.0, 0.0);
+    tc.kap = ke.x;
+    tc.eta = ke.y;
     tc.off = p.off;
     tc.magic = kMagic + (double)p.off;
     tc.s_max = p.s_max;
@@ -519,6 +523,7 @@ struct TrackTables {
     const double *dtab;    // [n_groups][n_pad][R]
     const double *A;       // [n_ap][n_P]
     const double2 *casa;   // [n_P][n_tasc]
+    const double2 *ke;     // [n_tasc] (e cos omega, e sin omega), or NULL (circular orbits)
     int n_pad, R;
     int n_pix, n_ap, n_P, n_tasc, n_f0;
     int64_t k_band0;
@@ -539,7 +544,7 @@ __device__ __forceinline__ TemplateCoord decode_template(const TrackTables &t, u
 }
 
 struct TemplateConst {
-    double A, CA, SA, u;
+    double A, CA, SA, u, kap, eta;
     const double2 *cs;
     const double *d;
     int d_stride, mj;
@@ -552,6 +557,9 @@ __device__ __forceinline__ TemplateConst template_const(const TrackTables &t, co
     const double2 q = t.casa[c.ip * t.n_tasc + c.it];
     k.CA = q.x;
     k.SA = q.y;
+    const double2 ke = t.ke ? t.ke[c.it] : make_double2(0.0, 0.0);
+    k.kap = ke.x;
+    k.eta = ke.y;
     k.u = (double)(t.k_band0 + c.j);
     k.cs = t.cs + (int64_t)c.ip * t.n_pad;
     k.d = t.dtab + ((int64_t)(c.pix / t.R) * t.n_pad) * t.R + (c.pix % t.R);
@@ -563,7 +571,7 @@ __device__ __forceinline__ TemplateConst template_const(const TrackTables &t, co
 __device__ __forceinline__ int track_column(const TemplateConst &k, int i, int n_bins)
 {
     const double2 cs = k.cs[i];
-    const double B = dmul(k.A, dadd(dmul(cs.x, k.CA), dmul(cs.y, k.SA)));
+    const double B = dmul(k.A, orbit_bracket(cs.x, cs.y, k.CA, k.SA, k.kap, k.eta));
     const double g = dsub(k.d[(int64_t)i * k.d_stride], B);
     const int col = shift_of(k.u, g, kMagic + (double)k.mj, k.mj);
     return (col >= 0 && col < n_bins) ? col : -1;

@@ -98,6 +98,7 @@ struct PixParams {
     const double *dpix;         // [n_pg][n_pad / 2][32][2]
     const double *A;            // [n_ap][n_P]
     const double2 *casa;        // [n_P][n_tasc]
+    const double2 *ke;          // [n_tasc] (e cos omega, e sin omega), or NULL (circular orbits)
     int n_pad, n_pos, n_chunks, n_stages;
     int n_pix, n_ap, n_P, n_tasc, n_f0;
     int j0, n_fj;               // f0 tile
@@ -379,9 +380,14 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
             mbar_wait(&full[st], parity);
             const unsigned char *sp = smem + kPixHeader + st * L.stride;
             const double2 *cs = reinterpret_cast<const double2 *>(sp + L.tab_bytes);
-            {   // binary terms of this stage: B = fl(A fl(fl(C CA) + fl(S SA)))  (R-5), one per lane
+            {   // binary terms of this stage: B = fl(A bracket)  (R-5, R-23), one per lane
                 const double2 c = cs[lane >> 1];
-                bbuf[lane] = __dmul_rn(A_d, __dadd_rn(__dmul_rn(c.x, q_d.x), __dmul_rn(c.y, q_d.y)));
+                if (p.ke) {                              // eccentric grid (Eq. 14): the pair is re-read per stage (L1), so
+                    const double2 ke_d = p.ke[rd ? it[1] : it[0]];   // that the circular search keeps its registers
+                    bbuf[lane] = __dmul_rn(A_d, orbit_bracket(c.x, c.y, q_d.x, q_d.y, ke_d.x, ke_d.y));
+                } else {
+                    bbuf[lane] = __dmul_rn(A_d, __dadd_rn(__dmul_rn(c.x, q_d.x), __dmul_rn(c.y, q_d.y)));
+                }
                 __syncwarp();                            // (the previous stage's readers passed the __syncwarp of pix_release)
             }
             const double2 *bpair = reinterpret_cast<const double2 *>(bbuf);
@@ -415,6 +421,8 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
                 tc.u0 = kc.u0; tc.uL = kc.uL; tc.magic = kMagic; tc.off = p.off; tc.s_max = p.s_max; tc.s_zero = p.s_zero;
                 tc.n_fj = p.n_fj;
                 tc.A = tcst[r * 4 + 0]; tc.CA = tcst[r * 4 + 1]; tc.SA = tcst[r * 4 + 2];
+                const double2 ke_r = p.ke ? p.ke[it[r]] : make_double2(0.0, 0.0);
+                tc.kap = ke_r.x; tc.eta = ke_r.y;
                 uint32_t tp[kFixPlanes][NW];
 #pragma unroll
                 for (int q = 0; q < kFixPlanes; ++q)

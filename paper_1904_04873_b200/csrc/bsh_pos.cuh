@@ -100,6 +100,7 @@ struct PosParams {
     const float *w_pad;         // [n_pad]
     const double *A;            // [n_ap][n_P]
     const double2 *casa;        // [n_P][n_tasc]
+    const double2 *ke;          // [n_tasc] (e cos omega, e sin omega), or NULL (circular orbits)
     int n_pad, n_pos, n_chunks, n_stages;
     int n_pix, n_ap, n_P, n_tasc, n_f0;
     int j0, n_fj;               // f0 tile
@@ -148,6 +149,9 @@ __device__ __forceinline__ TrackConst pos_track_const(const PosParams &p, const 
     const double2 q = p.casa[c.ip * p.n_tasc + c.it];
     tc.CA = q.x;
     tc.SA = q.y;
+    const double2 ke = p.ke ? p.ke[c.it] : make_double2(0.0, 0.0);
+    tc.kap = ke.x;
+    tc.eta = ke.y;
     tc.off = p.off;
     tc.magic = kMagic + (double)p.off;
     tc.s_max = p.s_max;

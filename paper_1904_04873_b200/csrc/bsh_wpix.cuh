@@ -112,6 +112,7 @@ struct WpixParams {
     const float *w_pad;         // [n_pad]
     const double *A;            // [n_ap][n_P]
     const double2 *casa;        // [n_P][n_tasc]
+    const double2 *ke;          // [n_tasc] (e cos omega, e sin omega), or NULL (circular orbits)
     int n_pad, n_pos, n_chunks, n_stages;
     int n_pix, n_ap, n_P, n_tasc, n_f0;
     int j0, n_fj;               // f0 tile
@@ -359,7 +360,13 @@ __global__ void __launch_bounds__(32 * kWpixWarps, 1) stage1_weighted_pix_kernel
             const unsigned char *sp = smem + kWpixHeader + st * L.stride;
             {   // binary terms of this stage: B = fl(A fl(fl(C CA) + fl(S SA)))  (R-5), lane l the one of SFT l & 15
                 const double2 c = reinterpret_cast<const double2 *>(sp + L.tab_bytes)[lane & (kStageSfts - 1)];
-                const double Bv = __dmul_rn(A_d, __dadd_rn(__dmul_rn(c.x, q_d.x), __dmul_rn(c.y, q_d.y)));
+                double Bv;
+                if (p.ke) {                              // eccentric grid (Eq. 14): the pair is re-read per stage (L1), so
+                    const double2 ke_d = p.ke[it];       // that the circular search keeps its registers
+                    Bv = __dmul_rn(A_d, orbit_bracket(c.x, c.y, q_d.x, q_d.y, ke_d.x, ke_d.y));
+                } else {
+                    Bv = __dmul_rn(A_d, __dadd_rn(__dmul_rn(c.x, q_d.x), __dmul_rn(c.y, q_d.y)));
+                }
                 __syncwarp();                            // the previous stage's readers are done with bwarp
                 if (lane < kStageSfts) bwarp[lane] = Bv;
                 __syncwarp();
@@ -393,7 +400,8 @@ __global__ void __launch_bounds__(32 * kWpixWarps, 1) stage1_weighted_pix_kernel
             TrackConst tc;
             tc.u0 = kc.u0; tc.uL = kc.uL; tc.magic = kMagic; tc.off = p.off; tc.s_max = p.s_max; tc.s_zero = p.s_zero;
             tc.n_fj = p.n_fj;
-            tc.A = A_d; tc.CA = q_d.x; tc.SA = q_d.y;
+            const double2 ke_f = p.ke ? p.ke[it] : make_double2(0.0, 0.0);
+            tc.A = A_d; tc.CA = q_d.x; tc.SA = q_d.y; tc.kap = ke_f.x; tc.eta = ke_f.y;
             for (int n = 0; n < npend; ++n) {
                 const int i = (int)list[n];
                 const double2 c = p.cs[(int64_t)ip * p.n_pad + i];

@@ -69,6 +69,7 @@ void run(int n_sft, int n_pix, int n_ap, int n_P, int n_tasc, int n_f0, int64_t 
                         tc.A = T.A[(size_t)ia * n_P + ip];
                         tc.CA = T.casa[((size_t)ip * n_tasc + it) * 2];
                         tc.SA = T.casa[((size_t)ip * n_tasc + it) * 2 + 1];
+                        tc.kap = 0.0; tc.eta = 0.0;
                         tc.off = (int)(k_band0 - k_slab0) + j0 + tg.off_table;
                         tc.magic = kMagic + (double)tc.off;
                         tc.s_max = tg.s_max;
@@ -180,6 +181,7 @@ void run_pix(int n_sft, int n_pix, int n_ap, int n_P, int n_tasc, int n_f0, int6
                         tc.A = T.A[(size_t)ia * n_P + ip];
                         tc.CA = T.casa[((size_t)ip * n_tasc + it) * 2];
                         tc.SA = T.casa[((size_t)ip * n_tasc + it) * 2 + 1];
+                        tc.kap = 0.0; tc.eta = 0.0;
                         tc.off = (int)(k_band0 - k_slab0) + j0 + pg.off_table;
                         tc.magic = kMagic + (double)tc.off;
                         tc.s_max = pg.s_max;
