@@ -25,6 +25,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import sys
 import threading
@@ -314,6 +315,9 @@ def main_ours(args, rank, local_rank, world):
         extras["config2"] = sub_config2(torch, bsh, ctx, timed, peaks)
         extras["config5_sweep"] = sweep_config5(torch, bsh, n_patches=32)
         extras["nc_fraction"] = sub_nc_fraction(torch, bsh, ctx)
+        extras["frontend"] = sub_frontend(torch, bsh, ctx, wl, flush)
+        extras["eccentric"] = sub_eccentric(torch, bsh, ctx, timed)
+        extras["postprocessing"] = sub_post(torch, bsh, ctx)
 
     kinds = {names[head_mode]: (k_ms, total_ms / args.steps, st), names[other_mode]: (ok_ms, o_total_ms / o_steps, st_o)}
     roof = {m: roofline(m, wl, kinds[m][0], kinds[m][2], peaks) for m in kinds}
@@ -495,6 +499,65 @@ def sub_nc_fraction(torch, bsh, ctx):
                "n_passes": st["n_passes"]}
         del d_top
     return res
+
+
+def sub_frontend(torch, bsh, ctx, wl, flush):
+    """SURVEY NEXT-2 (Eq. 20-21): complex SFT bins -> 101-bin running-median normalised power ->
+    peakgram, one fused kernel, at the size of the headline patch.  HBM-bound by its algorithmic bytes (8 B per raw bin in,
+    4 B per power + 1 bit per peak out); reported against the measured HBM copy bandwidth."""
+    window = 101
+    raw = synth.raw_sft_bins(31, wl.n_sft, wl.n_bins + window - 1)
+    d_raw = torch.from_numpy(raw).cuda()
+    ms = []
+    for _ in range(6):
+        flush.fill_(1)
+        ctx.normalise_peakgram(d_raw, window=window)
+        ms.append(ctx.stats()["frontend_ms"])
+    t = float(np.median(ms[1:]))
+    n, n_raw, k = wl.n_sft, raw.shape[1], wl.n_bins
+    algo_bytes = 8 * n * n_raw + 4 * n * k + 4 * n * ((k + 31) // 32)
+    hbm = measured_peaks_file().get("hbm_gbs")
+    return {"workload": f"{n} SFTs x {n_raw} raw complex bins -> {k} slab columns, running median over {window} bins",
+            "kernel": "normalise_peakgram_kernel", "kernel_ms": t, "algorithmic_bytes": algo_bytes,
+            "roofline": {"bound": "hbm", "achieved": algo_bytes / (t * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                         "frac": (algo_bytes / (t * 1e-3) / 1e9 / hbm) if hbm else None,
+                         "note": "the per-row sort and median scan are on-chip work above the HBM floor; the kernel runs once "
+                                 "per band, in front of ~50 sky patches (L451)"}}
+
+
+def sub_eccentric(torch, bsh, ctx, timed):
+    """SURVEY NEXT-3 (Eq. 14): config 2 with every template on an eccentric orbit (one pair e cos w, e sin w != 0,
+    so the template count is unchanged): the accumulation kernel's time against the circular search."""
+    import dataclasses
+    wl = synth.config2()
+    wle = dataclasses.replace(wl, ecosw=np.array([0.03 * math.cos(0.7)]), esinw=np.array([0.03 * math.sin(0.7)]))
+    out = {"workload": "config 2, every template with (e cos w, e sin w) = 0.03 (cos 0.7, sin 0.7)"}
+    for name, w in (("circular", wl), ("eccentric", wle)):
+        patch = Patch(torch, bsh, ctx, w)
+        for mode, mname in ((bsh.BSH_UNWEIGHTED, "unweighted"), (bsh.BSH_WEIGHTED, "weighted")):
+            _, k_ms, _, _ = timed(lambda: patch.step(mode), 5, 2)
+            out[f"{name}_{mname}_kernel_ms"] = k_ms
+    return out
+
+
+def sub_post(torch, bsh, ctx):
+    """SURVEY NEXT-4 (section V.E, Eq. 44): 5000 candidates (L496) -> clusters + centroids; two lists -> coincidences."""
+    a, b = synth.candidate_list(41, n_background=4900, chain=40), synth.candidate_list(42, n_background=4900)
+    da = tuple(torch.from_numpy(x).cuda() for x in (a.param, a.res, a.sig))
+    db = tuple(torch.from_numpy(x).cuda() for x in (b.param, b.res, b.sig))
+    out = {"workload": f"{a.n} candidates: clustering window sqrt(14) bins; {a.n} x {b.n} coincidences, window 3 bins (L511)"}
+    for rep in range(2):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        c = ctx.post_cluster(da, math.sqrt(14.0))
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        pa, _, _, _ = ctx.post_coincidences(da, db, 3.0)
+        torch.cuda.synchronize()
+        t2 = time.perf_counter()
+        out.update({"cluster_ms": (t1 - t0) * 1e3, "n_clusters": int(c["root"].numel()), "coincidences_ms": (t2 - t1) * 1e3,
+                    "n_pairs": int(pa.numel()), "pair_distances_per_s": (a.n * a.n) / max(t1 - t0, 1e-9)})
+    return out
 
 
 def main_config5(args, rank, world, torch, bsh, ctx, dist, peaks):

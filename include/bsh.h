@@ -202,6 +202,36 @@ int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, c
 int bsh_search_patch_host(bsh_ctx *ctx, const float *h_rho, const float *h_w, float rho_th, const bsh_sfts *sfts,
                           const bsh_grid *grid, int32_t mode, int32_t topk, bsh_cand *h_top, int32_t *h_n_top);
 
+/* Post-processing of the toplists (section V.E).  A candidate set: n points
+ * p = (f, x, y, a_p, Omega, t_asc) (x, y: ecliptic coordinates projected into the ecliptic plane, L397), the parameter
+ * resolutions at each point in the same order (delta f, delta theta, delta theta, delta a_p, delta Omega, delta t_asc:
+ * Eq. 30-33), and a significance per point.  Distance (Eq. 44, "a mean of the resolution at both points" L399):
+ *     d^2(a, b) = sum_k [ (p_k(a) - p_k(b)) / ((delta_k(a) + delta_k(b)) / 2) ]^2
+ * in FP64, one rounding per operation, the six squares added in the order of Eq. (44) (reading R-25: plain differences,
+ * t_asc is not wrapped modulo P).  Both calls are synchronous; n <= 32768. */
+typedef struct {
+    int32_t       n;
+    const double *d_param;   /* [n][6] */
+    const double *d_res;     /* [n][6], all > 0 */
+    const double *d_sig;     /* [n]    */
+} bsh_candset;
+
+/* Step 1 (L387-L393): every pair (a in A, b in B) with d(a, b) < window, in (a, b) lexicographic order: indices, the
+ * significance-weighted centroid [6] and the summed significance of each pair.  At most max_pairs are written;
+ * *h_n_pairs receives the number found (may exceed max_pairs: call again with larger buffers). */
+int bsh_post_coincidences(bsh_ctx *ctx, const bsh_candset *a, const bsh_candset *b, double window, int64_t max_pairs,
+                          int32_t *d_pair_a, int32_t *d_pair_b, double *d_centroid, double *d_pair_sig, int64_t *h_n_pairs);
+
+/* Steps 2-3 (L401-L405): clusters = connected components of the graph d < window; d_label[i] = smallest index of the
+ * members of i's cluster.  prune_window > 0 (option B, L403): members at that distance or further from the cluster's top
+ * template (largest significance, smallest index among equals) are removed, d_label = -1.  Per cluster, in increasing
+ * label order ([n] arrays, *h_n_clusters entries written): d_root (the label), d_centroid [6] (significance-weighted
+ * average of the members, taken in index order), d_cluster_sig (summed significance), d_n_members.  *h_best = position
+ * of the most significant cluster (first among equals), the one kept per 0.1 Hz band (L405); -1 when n = 0. */
+int bsh_post_cluster(bsh_ctx *ctx, const bsh_candset *c, double window, double prune_window, int32_t *d_label,
+                     int32_t *d_root, double *d_centroid, double *d_cluster_sig, int32_t *d_n_members,
+                     int32_t *h_n_clusters, int32_t *h_best);
+
 /* Template index helpers (R-11).  Pure host functions.  The first pair is for circular grids (n_ecc = 0; on an eccentric
  * grid it addresses pair ie = 0 / drops ie); the _ecc pair carries the eccentricity index. */
 uint64_t bsh_template_index(const bsh_grid *grid, int32_t pix, int32_t ia, int32_t ip, int32_t it, int32_t j);

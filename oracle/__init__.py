@@ -54,6 +54,9 @@ def lib():
         _lib.orc_toplist.restype = C.c_int64
         _lib.orc_max_threads.restype = C.c_int
         _lib.orc_median_bias.restype = C.c_double
+        _lib.orc_distance2.restype = C.c_double
+        _lib.orc_coincidences.restype = C.c_int64
+        _lib.orc_cluster.restype = C.c_int32
     return _lib
 
 
@@ -213,3 +216,49 @@ def significance_count(nw, w, p=P_PEAK):
 def significance_power(pw, w):
     w = np.asarray(w, np.float64)
     return (np.asarray(pw, np.float64) - w.sum()) / math.sqrt((w * w).sum())
+
+
+# --- post-processing of the toplists (section V.E, Eq. 44) ---------------------------
+NPAR = 6                                         # (f, x, y, a_p, Omega, t_asc), the order of Eq. (44)
+
+
+def _cand(p, r, s):
+    p, r, s = _f64(p), _f64(r), _f64(s)
+    assert p.ndim == 2 and p.shape[1] == NPAR and r.shape == p.shape and s.shape == (p.shape[0],)
+    return p, r, s
+
+
+def distance2(pa, ra, pb, rb) -> float:
+    """Eq. (44): squared parameter-space distance in bins, mean of the two points' resolutions (L399)."""
+    pa, ra, pb, rb = (_f64(x) for x in (pa, ra, pb, rb))
+    return float(lib().orc_distance2(C.c_void_p(pa.ctypes.data), C.c_void_p(ra.ctypes.data), C.c_void_p(pb.ctypes.data),
+                                     C.c_void_p(rb.ctypes.data)))
+
+
+def coincidences(pa, ra, sa, pb, rb, sb, window):
+    """Step 1 (L387-L393): pairs closer than `window`, (a, b) order.  -> (pair_a, pair_b, centroid [n, 6], significance)."""
+    pa, ra, sa = _cand(pa, ra, sa)
+    pb, rb, sb = _cand(pb, rb, sb)
+    cap = max(1, pa.shape[0] * pb.shape[0])
+    ia, ib = np.zeros(cap, np.int32), np.zeros(cap, np.int32)
+    cen, sig = np.zeros((cap, NPAR), np.float64), np.zeros(cap, np.float64)
+    v = lambda a: C.c_void_p(a.ctypes.data)
+    n = lib().orc_coincidences(C.c_int32(pa.shape[0]), v(pa), v(ra), v(sa), C.c_int32(pb.shape[0]), v(pb), v(rb), v(sb),
+                               C.c_double(window), C.c_int64(cap), v(ia), v(ib), v(cen), v(sig))
+    return ia[:n].copy(), ib[:n].copy(), cen[:n].copy(), sig[:n].copy()
+
+
+def cluster(p, r, s, window, prune_window=0.0):
+    """Steps 2-3 (L401-L405).  -> dict(label [n] (smallest member index, -1 pruned), root, centroid, significance,
+    n_members (per cluster, increasing label), best (position of the most significant cluster or -1))."""
+    p, r, s = _cand(p, r, s)
+    n = p.shape[0]
+    label = np.zeros(max(n, 1), np.int32)
+    root, members = np.zeros(max(n, 1), np.int32), np.zeros(max(n, 1), np.int32)
+    cen, sig = np.zeros((max(n, 1), NPAR), np.float64), np.zeros(max(n, 1), np.float64)
+    best = C.c_int32(-1)
+    v = lambda a: C.c_void_p(a.ctypes.data)
+    nc = lib().orc_cluster(C.c_int32(n), v(p), v(r), v(s), C.c_double(window), C.c_double(prune_window), v(label), v(root),
+                           v(cen), v(sig), v(members), C.byref(best))
+    return dict(label=label[:n].copy(), root=root[:nc].copy(), centroid=cen[:nc].copy(), significance=sig[:nc].copy(),
+                n_members=members[:nc].copy(), best=int(best.value))

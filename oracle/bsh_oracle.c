@@ -480,3 +480,126 @@ void orc_normalise(const float *sft, int32_t n_sft, int32_t n_raw, int32_t windo
     free(p);
     free(win);
 }
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Post-processing of the toplists, section V.E, L385-L407.
+ *
+ * A candidate is a point p = (f, x, y, a_p, Omega, t_asc) (x, y: "cartesian ecliptical coordinates projected into the
+ * ecliptical plane", L397) with a significance s and the parameter resolutions delta = (df, dtheta, dtheta, da_p, dOmega,
+ * dt_asc) AT that point.  Distance, Eq. (44), "given as a number of bins"; "we use a mean of the resolution at both
+ * points" (L399):
+ *     d^2(a, b) = sum_k [ (p_k(a) - p_k(b)) / ((delta_k(a) + delta_k(b)) / 2) ]^2        k in the order of Eq. (44)
+ * (R-25: plain differences, no wrap of t_asc modulo P; every operation one rounded FP64 operation in the order
+ * written, the six squares added left to right.)
+ *   coincidences (step 1, L387-L393): all pairs (a in list A, b in list B) with d < window; per pair the centroid
+ *       "average locations in parameter space weighted by significance" and the summed significance (R-25).
+ *   clusters (step 2, L401-L403): "analyzing the distance of each template from all other templates, and keeping a list of
+ *       indices of members with distances below the threshold ... if a template was already in a cluster its newly
+ *       generated cluster and the old one will be joined" = connected components of the graph d < window.  The label of a
+ *       cluster is the smallest index of its members.  Option B (L403): members further than prune_window from the
+ *       cluster's top template (largest significance, smallest index among equals) are removed (label -1).
+ *   centroids (step 3, L405): significance-weighted average of the members, summed significance; the most significant
+ *       cluster is the one kept per band.
+ * ------------------------------------------------------------------------------------------------------- */
+#define ORC_NPAR 6
+
+double orc_distance2(const double *pa, const double *ra, const double *pb, const double *rb)
+{
+    double d2 = 0.0;
+    for (int k = 0; k < ORC_NPAR; ++k) {
+        const double sum = ra[k] + rb[k];
+        const double res = 0.5 * sum;                      /* mean of the resolutions at both points, L399 */
+        const double diff = pa[k] - pb[k];
+        const double q = diff / res;
+        const double sq = q * q;
+        d2 = d2 + sq;                                      /* Eq. (44) */
+    }
+    return d2;
+}
+
+/* step 1: pairs in (a, b) lexicographic order; returns the number found (writes at most max_pairs) */
+int64_t orc_coincidences(int32_t na, const double *pa, const double *ra, const double *sa, int32_t nb, const double *pb,
+                         const double *rb, const double *sb, double window, int64_t max_pairs, int32_t *pair_a,
+                         int32_t *pair_b, double *centroid, double *pair_sig)
+{
+    int64_t n = 0;
+    const double w2 = window * window;
+    for (int32_t a = 0; a < na; ++a)
+        for (int32_t b = 0; b < nb; ++b) {
+            const double d2 = orc_distance2(pa + ORC_NPAR * (size_t)a, ra + ORC_NPAR * (size_t)a, pb + ORC_NPAR * (size_t)b,
+                                            rb + ORC_NPAR * (size_t)b);
+            if (!(d2 < w2)) continue;
+            if (n < max_pairs) {
+                pair_a[n] = a;
+                pair_b[n] = b;
+                const double s = sa[a] + sb[b];
+                pair_sig[n] = s;
+                for (int k = 0; k < ORC_NPAR; ++k) {
+                    const double wa = sa[a] * pa[ORC_NPAR * (size_t)a + k];
+                    const double wb = sb[b] * pb[ORC_NPAR * (size_t)b + k];
+                    centroid[ORC_NPAR * n + k] = (wa + wb) / s;
+                }
+            }
+            n += 1;
+        }
+    return n;
+}
+
+/* steps 2 and 3.  label[n]; per cluster (in increasing label order): root, centroid[6], summed significance, members.
+ * Returns the number of clusters; *best = position (in that order) of the most significant cluster, -1 if none. */
+int32_t orc_cluster(int32_t n, const double *p, const double *r, const double *s, double window, double prune_window,
+                    int32_t *label, int32_t *root, double *centroid, double *cluster_sig, int32_t *n_members, int32_t *best)
+{
+    const double w2 = window * window;
+    for (int32_t i = 0; i < n; ++i) label[i] = i;                       /* every template starts as its own cluster */
+    for (int32_t i = 0; i < n; ++i)
+        for (int32_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            const double d2 = orc_distance2(p + ORC_NPAR * (size_t)i, r + ORC_NPAR * (size_t)i, p + ORC_NPAR * (size_t)j,
+                                            r + ORC_NPAR * (size_t)j);
+            if (d2 < w2 && label[i] != label[j]) {                      /* join the two clusters (L401) */
+                const int32_t keep = label[i] < label[j] ? label[i] : label[j];
+                const int32_t drop = label[i] < label[j] ? label[j] : label[i];
+                for (int32_t m = 0; m < n; ++m)
+                    if (label[m] == drop) label[m] = keep;
+            }
+        }
+    if (prune_window > 0.0) {                                           /* option B, L403 */
+        const double pw2 = prune_window * prune_window;
+        int32_t *top = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+        for (int32_t c = 0; c < n; ++c) {
+            top[c] = -1;
+            for (int32_t m = 0; m < n; ++m)
+                if (label[m] == c && (top[c] < 0 || s[m] > s[top[c]])) top[c] = m;
+        }
+        for (int32_t m = 0; m < n; ++m) {
+            const int32_t t = top[label[m]];
+            const double d2 = orc_distance2(p + ORC_NPAR * (size_t)m, r + ORC_NPAR * (size_t)m, p + ORC_NPAR * (size_t)t,
+                                            r + ORC_NPAR * (size_t)t);
+            if (!(d2 < pw2) && m != t) label[m] = -(label[m] + 2);      /* marked; resolved below (labels stay readable) */
+        }
+        for (int32_t m = 0; m < n; ++m)
+            if (label[m] < 0) label[m] = -1;
+        free(top);
+    }
+    int32_t nc = 0;
+    *best = -1;
+    for (int32_t c = 0; c < n; ++c) {                                   /* clusters in increasing label order */
+        double ssum = 0.0, acc[ORC_NPAR] = {0, 0, 0, 0, 0, 0};
+        int32_t members = 0;
+        for (int32_t m = 0; m < n; ++m)
+            if (label[m] == c) {
+                members += 1;
+                ssum = ssum + s[m];
+                for (int k = 0; k < ORC_NPAR; ++k) acc[k] = acc[k] + s[m] * p[ORC_NPAR * (size_t)m + k];
+            }
+        if (members == 0) continue;
+        root[nc] = c;
+        n_members[nc] = members;
+        cluster_sig[nc] = ssum;
+        for (int k = 0; k < ORC_NPAR; ++k) centroid[ORC_NPAR * (size_t)nc + k] = acc[k] / ssum;   /* L405 */
+        if (*best < 0 || ssum > cluster_sig[*best]) *best = nc;
+        nc += 1;
+    }
+    return nc;
+}

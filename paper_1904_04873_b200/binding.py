@@ -16,7 +16,7 @@ BSH_FAMILY_AUTO, BSH_FAMILY_PIXEL_LANE, BSH_FAMILY_TEMPLATE_LANE, BSH_FAMILY_WIN
 EXPORTS = ["bsh_version", "bsh_create", "bsh_destroy", "bsh_last_error", "bsh_get_stats", "bsh_set_option",
            "bsh_measure_peaks", "bsh_build_peakgram", "bsh_normalise_peakgram", "bsh_median_bias",
            "bsh_stage1_hough", "bsh_stage1_launch", "bsh_stage1_collect", "bsh_stage2_power", "bsh_search_patch_host",
-           "bsh_template_index", "bsh_template_decode", "bsh_template_index_ecc", "bsh_template_decode_ecc"]
+           "bsh_template_index", "bsh_template_decode", "bsh_template_index_ecc", "bsh_template_decode_ecc", "bsh_post_coincidences", "bsh_post_cluster"]
 
 # numpy view of bsh_cand (24 bytes)
 CAND_DTYPE = np.dtype([("index", "<u8"), ("count", "<i4"), ("wcount", "<f4"), ("power", "<f4"), ("flags", "<u4")])
@@ -36,6 +36,10 @@ class _Grid(C.Structure):
                 ("n_f0", C.c_int32), ("n_ap", C.c_int32), ("h_ap", C.c_void_p), ("n_P", C.c_int32), ("h_P", C.c_void_p),
                 ("n_tasc", C.c_int32), ("h_tasc_frac", C.c_void_p),
                 ("n_ecc", C.c_int32), ("h_ecosw", C.c_void_p), ("h_esinw", C.c_void_p)]
+
+
+class _CandSet(C.Structure):
+    _fields_ = [("n", C.c_int32), ("d_param", C.c_void_p), ("d_res", C.c_void_p), ("d_sig", C.c_void_p)]
 
 
 class Stats(C.Structure):
@@ -243,6 +247,54 @@ class Context:
                                                    C.byref(pb.sfts), C.byref(pb.grid), C.c_int32(mode), C.c_int32(topk),
                                                    C.c_void_p(out.ctypes.data), C.byref(n_top)))
         return out, int(n_top.value)
+
+    # ---- post-processing of the toplists (section V.E) -------------------------------------------------------------
+    def _candset(self, d_param, d_res, d_sig):
+        torch = self.torch
+        n = int(d_param.shape[0])
+        for t, shape in ((d_param, (n, 6)), (d_res, (n, 6)), (d_sig, (n,))):
+            assert t.is_cuda and t.dtype == torch.float64 and tuple(t.shape) == shape and t.is_contiguous()
+        return _CandSet(n=n, d_param=d_param.data_ptr() if n else None, d_res=d_res.data_ptr() if n else None,
+                        d_sig=d_sig.data_ptr() if n else None)
+
+    def post_coincidences(self, a, b, window: float, max_pairs=None):
+        """a, b: (d_param [n, 6], d_res [n, 6], d_sig [n]) CUDA float64 tensors.  Returns (pair_a, pair_b, centroid [m, 6],
+        significance [m]) CUDA tensors, pairs in (a, b) order (Eq. 44)."""
+        torch = self.torch
+        ca, cb = self._candset(*a), self._candset(*b)
+        cap = int(max_pairs if max_pairs is not None else max(1, min(ca.n * cb.n, 1 << 22)))
+        while True:
+            pa = torch.empty(cap, dtype=torch.int32, device="cuda")
+            pb = torch.empty(cap, dtype=torch.int32, device="cuda")
+            cen = torch.empty((cap, 6), dtype=torch.float64, device="cuda")
+            sig = torch.empty(cap, dtype=torch.float64, device="cuda")
+            n = C.c_int64(0)
+            self._check(self.lib.bsh_post_coincidences(self._ctx, C.byref(ca), C.byref(cb), C.c_double(window), C.c_int64(cap),
+                                                       C.c_void_p(pa.data_ptr()), C.c_void_p(pb.data_ptr()),
+                                                       C.c_void_p(cen.data_ptr()), C.c_void_p(sig.data_ptr()), C.byref(n)))
+            if n.value <= cap or max_pairs is not None:
+                m = min(n.value, cap)
+                return pa[:m], pb[:m], cen[:m], sig[:m]
+            cap = int(n.value)
+
+    def post_cluster(self, cands, window: float, prune_window: float = 0.0):
+        """cands: (d_param, d_res, d_sig).  Returns dict(label [n], root, centroid [c, 6], significance, n_members, best)."""
+        torch = self.torch
+        c = self._candset(*cands)
+        n = max(c.n, 1)
+        label = torch.empty(n, dtype=torch.int32, device="cuda")
+        root = torch.empty(n, dtype=torch.int32, device="cuda")
+        members = torch.empty(n, dtype=torch.int32, device="cuda")
+        cen = torch.empty((n, 6), dtype=torch.float64, device="cuda")
+        sig = torch.empty(n, dtype=torch.float64, device="cuda")
+        nc, best = C.c_int32(0), C.c_int32(-1)
+        self._check(self.lib.bsh_post_cluster(self._ctx, C.byref(c), C.c_double(window), C.c_double(prune_window),
+                                              C.c_void_p(label.data_ptr()), C.c_void_p(root.data_ptr()),
+                                              C.c_void_p(cen.data_ptr()), C.c_void_p(sig.data_ptr()),
+                                              C.c_void_p(members.data_ptr()), C.byref(nc), C.byref(best)))
+        k = nc.value
+        return dict(label=label[:c.n], root=root[:k], centroid=cen[:k], significance=sig[:k], n_members=members[:k],
+                    best=int(best.value))
 
     def set_option(self, option: int, value: int):
         """Diagnostic switches (kernel family, table geometry); see include/bsh.h."""

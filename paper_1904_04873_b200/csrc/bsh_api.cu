@@ -20,6 +20,7 @@
 #include "bsh_wpix.cuh"
 #include "bsh_peaks.cuh"
 #include "bsh_frontend.cuh"
+#include "bsh_post.cuh"
 
 using namespace bsh;
 
@@ -85,6 +86,7 @@ struct bsh_ctx {
     Pending pend;
     int opt_family = BSH_FAMILY_AUTO, opt_force_clamp = 0, opt_pixels_per_thread = 0;   // bsh_set_option
     DevBuf peak_samples;
+    DevBuf post_adj, post_cnt, post_off, post_tmp;
     bsh_stats st = {};
     bool have_front = false;
     bool have_pk = false, have_setup = false, have_kernel = false, have_select = false, have_s2 = false;
@@ -636,7 +638,8 @@ int bsh_destroy(bsh_ctx *ctx)
     const DeviceGuard device_guard(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     DevBuf *bufs[] = {&ctx->wtab, &ctx->w_pad, &ctx->stats, &ctx->thr, &ctx->dtab, &ctx->nvec, &ctx->cand, &ctx->cand_count,
-                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->psplit, &ctx->tab7, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top, &ctx->peak_samples};
+                      &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->psplit, &ctx->tab7, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top, &ctx->peak_samples,
+                      &ctx->post_adj, &ctx->post_cnt, &ctx->post_off, &ctx->post_tmp};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto &c : ctx->cache) {
@@ -1135,6 +1138,98 @@ int bsh_search_patch_host(bsh_ctx *ctx, const float *h_rho, const float *h_w, fl
     TRY(bsh_stage2_power(ctx, (const float *)ctx->h_rho.p, K, &s, grid, (bsh_cand *)ctx->h_top.p, *h_n_top, 1));
     CK(cudaMemcpyAsync(h_top, ctx->h_top.p, sizeof(bsh_cand) * (size_t)topk, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
+    return BSH_OK;
+}
+
+static int check_candset(bsh_ctx *ctx, const bsh_candset *c, const char *what)
+{
+    if (!c || c->n < 0 || c->n > 32768 || (c->n > 0 && (!c->d_param || !c->d_res || !c->d_sig)))
+        return fail(ctx, BSH_EINVAL, "%s: bad candidate set", what);
+    return BSH_OK;
+}
+
+int bsh_post_coincidences(bsh_ctx *ctx, const bsh_candset *a, const bsh_candset *b, double window, int64_t max_pairs,
+                          int32_t *d_pair_a, int32_t *d_pair_b, double *d_centroid, double *d_pair_sig, int64_t *h_n_pairs)
+{
+    if (!ctx) return BSH_EINVAL;
+    TRY(check_candset(ctx, a, "bsh_post_coincidences"));
+    TRY(check_candset(ctx, b, "bsh_post_coincidences"));
+    if (!h_n_pairs || max_pairs < 0 || !(window > 0.0) || (max_pairs > 0 && (!d_pair_a || !d_pair_b || !d_centroid || !d_pair_sig)))
+        return fail(ctx, BSH_EINVAL, "bsh_post_coincidences: bad arguments");
+    *h_n_pairs = 0;
+    if (a->n == 0 || b->n == 0) return BSH_OK;
+    const DeviceGuard device_guard(ctx->device);
+    const int words = (b->n + 31) / 32;
+    TRY(ensure(ctx, ctx->post_adj, (size_t)a->n * words * 4));
+    TRY(ensure(ctx, ctx->post_cnt, (size_t)a->n * 4));
+    TRY(ensure(ctx, ctx->post_off, (size_t)(a->n + 1) * 8));
+    CK(cudaMemsetAsync(ctx->post_cnt.p, 0, (size_t)a->n * 4, ctx->stream));
+    const int64_t warps = (int64_t)a->n * words;
+    post_adjacency_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, ctx->stream>>>(
+        a->n, a->d_param, a->d_res, b->n, b->d_param, b->d_res, window * window, 0, words, (uint32_t *)ctx->post_adj.p,
+        (int32_t *)ctx->post_cnt.p);
+    post_scan_kernel<<<1, 1024, 0, ctx->stream>>>(a->n, (const int32_t *)ctx->post_cnt.p, (int64_t *)ctx->post_off.p);
+    post_pairs_kernel<<<(a->n + 255) / 256, 256, 0, ctx->stream>>>(
+        a->n, words, (const uint32_t *)ctx->post_adj.p, (const int64_t *)ctx->post_off.p, a->d_param, a->d_sig, b->d_param,
+        b->d_sig, max_pairs, d_pair_a, d_pair_b, d_centroid, d_pair_sig);
+    count_launch(ctx, 3);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(h_n_pairs, (const int64_t *)ctx->post_off.p + a->n, 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return BSH_OK;
+}
+
+int bsh_post_cluster(bsh_ctx *ctx, const bsh_candset *c, double window, double prune_window, int32_t *d_label,
+                     int32_t *d_root, double *d_centroid, double *d_cluster_sig, int32_t *d_n_members,
+                     int32_t *h_n_clusters, int32_t *h_best)
+{
+    if (!ctx) return BSH_EINVAL;
+    TRY(check_candset(ctx, c, "bsh_post_cluster"));
+    if (!h_n_clusters || !h_best || !(window > 0.0)) return fail(ctx, BSH_EINVAL, "bsh_post_cluster: bad arguments");
+    *h_n_clusters = 0;
+    *h_best = -1;
+    const int n = c->n;
+    if (n == 0) return BSH_OK;
+    if (!d_label || !d_root || !d_centroid || !d_cluster_sig || !d_n_members) return fail(ctx, BSH_EINVAL, "bsh_post_cluster: null output");
+    const DeviceGuard device_guard(ctx->device);
+    const int words = (n + 31) / 32;
+    TRY(ensure(ctx, ctx->post_adj, (size_t)n * words * 4));
+    // scratch: [flag + (n_clusters, best)] | top [n] | members_by_label [n] | sig_by_label [n] | cen_by_label [6 n]
+    TRY(ensure(ctx, ctx->post_tmp, 64 + (size_t)n * (4 + 4 + 8 + 8 * kNPar)));
+    int *d_flag = (int *)ctx->post_tmp.p;
+    int32_t *d_top = (int32_t *)((char *)ctx->post_tmp.p + 64);
+    int32_t *d_mem = d_top + n;
+    double *d_sigl = (double *)((char *)ctx->post_tmp.p + 64 + (size_t)n * 8);
+    double *d_cenl = d_sigl + n;
+    const int64_t warps = (int64_t)n * words;
+    post_adjacency_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, ctx->stream>>>(
+        n, c->d_param, c->d_res, n, c->d_param, c->d_res, window * window, 1, words, (uint32_t *)ctx->post_adj.p, nullptr);
+    post_iota_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(n, d_label);
+    count_launch(ctx, 2);
+    for (int iter = 0; iter < n + 2; ++iter) {               // min-label propagation: at most (diameter + 1) sweeps
+        CK(cudaMemsetAsync(d_flag, 0, 4, ctx->stream));
+        post_propagate_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(n, words, (const uint32_t *)ctx->post_adj.p, d_label,
+                                                                       d_flag);
+        count_launch(ctx);
+        CK(cudaMemcpyAsync(ctx->pinned_count + 8, d_flag, 4, cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+        if (ctx->pinned_count[8] == 0) break;
+    }
+    if (prune_window > 0.0) {
+        post_top_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(n, d_label, c->d_sig, d_top);
+        post_prune_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(n, c->d_param, c->d_res, d_top,
+                                                                   prune_window * prune_window, d_label);
+        count_launch(ctx, 2);
+    }
+    post_centroid_kernel<<<(n + 127) / 128, 128, 0, ctx->stream>>>(n, c->d_param, c->d_sig, d_label, d_cenl, d_sigl, d_mem);
+    post_compact_kernel<<<1, 1024, 0, ctx->stream>>>(n, d_cenl, d_sigl, d_mem, d_root, d_centroid, d_cluster_sig, d_n_members,
+                                                     (int32_t *)d_flag + 2);
+    count_launch(ctx, 2);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(ctx->pinned_count + 8, (int32_t *)d_flag + 2, 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    *h_n_clusters = (int32_t)ctx->pinned_count[8];
+    *h_best = (int32_t)ctx->pinned_count[9];
     return BSH_OK;
 }
 

@@ -440,3 +440,62 @@ def overlapped_stage2_set(wl: Workload, seed: int = 0, lat_deg: float = 30.6, th
     v2 = detector_velocity_over_c(t2, lat_deg, theta0)
     return dataclasses.replace(wl, name=wl.name + "-stage2", t_mid=np.ascontiguousarray(t2), v_over_c=v2,
                                rho=exp_powers(rng, n2, wl.n_bins), w=lognormal_weights(rng, n2))
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# Candidate lists for the post-processing (section V.E): toplist entries as points of parameter space with
+# the resolutions of Eq. 30-33 at each point.  Inputs only: no distance, no clustering here.
+# ----------------------------------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class Candidates:
+    param: np.ndarray            # [n, 6] f64: f [Hz], x, y (ecliptic plane), a_p [s], Omega [rad/s], t_asc [s]
+    res: np.ndarray              # [n, 6] f64: delta f, delta theta, delta theta, delta a_p, delta Omega, delta t_asc
+    sig: np.ndarray              # [n] f64 significance
+    truth: np.ndarray            # [n] int: index of the planted group the candidate was drawn around, -1 = background
+
+    @property
+    def n(self) -> int:
+        return int(self.param.shape[0])
+
+
+def resolutions(f, ap, Om, t_sft=900.0, t_obs=60 * DAY, m_a=0.4, m_om=0.4, m_t=0.4, pixel_factor=1.0) -> np.ndarray:
+    """Eq. 30-33 (L270-L290) at the given points: [.., 6] = (1/T, dTheta, dTheta, d a_p, d Omega, d t_asc)."""
+    f, ap, Om = (np.asarray(v, np.float64) for v in (f, ap, Om))
+    dth = C_LIGHT / (V_ORB * t_sft * f * pixel_factor)
+    da = math.sqrt(6 * m_a) / (math.pi * t_sft * f * Om)
+    dom = math.sqrt(72 * m_om) / (math.pi * t_sft * f * ap * Om * t_obs)
+    dt = math.sqrt(6 * m_t) / (math.pi * t_sft * f * ap * Om ** 2)
+    return np.stack([np.full_like(f, 1.0 / t_sft), dth, dth, da, dom, dt], -1)
+
+
+def candidate_list(seed: int, n_background: int = 300, groups=((12, 0.8), (7, 0.8), (20, 1.5)), f_band=(150.0, 150.1),
+                   chain: int = 0) -> Candidates:
+    """A toplist-like set of points: `n_background` isolated candidates spread over the band / patch / binary ranges of
+    config 2, plus planted groups (n_members, spread in bins) scattered around seeded centres (what a signal or a line
+    leaves in a toplist), plus optionally a `chain` of points 0.9 bins apart (a cluster held together by single links).
+    Significances: exponential background, louder group members."""
+    rng = _rng(seed, 909)
+    lo = np.array([f_band[0], -0.02, -0.02, 10.0, 2 * math.pi / (45 * DAY), 0.0])
+    hi = np.array([f_band[1], 0.02, 0.02, 40.0, 2 * math.pi / (15 * DAY), 15 * DAY])
+    pts = [lo + (hi - lo) * rng.random((n_background, 6))]
+    truth = [np.full(n_background, -1)]
+    sig = [5.0 + rng.standard_exponential(n_background)]
+    for g, (members, spread) in enumerate(groups):
+        c = lo + (hi - lo) * (0.2 + 0.6 * rng.random(6))
+        r = resolutions(c[0], c[3], c[4])
+        pts.append(c + spread / math.sqrt(6.0) * r * rng.standard_normal((members, 6)))
+        truth.append(np.full(members, g))
+        sig.append(8.0 + 4.0 * rng.random(members))
+    if chain:
+        c = lo + (hi - lo) * 0.5
+        r = resolutions(c[0], c[3], c[4])
+        step = np.zeros(6)
+        step[0] = 0.9 * r[0]
+        pts.append(c + np.arange(chain)[:, None] * step)
+        truth.append(np.full(chain, len(groups)))
+        sig.append(6.0 + rng.random(chain))
+    param = np.concatenate(pts)
+    order = rng.permutation(param.shape[0])
+    param = np.ascontiguousarray(param[order])
+    return Candidates(param=param, res=np.ascontiguousarray(resolutions(param[:, 0], param[:, 3], param[:, 4])),
+                      sig=np.ascontiguousarray(np.concatenate(sig)[order]), truth=np.concatenate(truth)[order])
