@@ -529,9 +529,10 @@ def sub_eccentric(torch, bsh, ctx, timed):
     """SURVEY NEXT-3 (Eq. 14): config 2 with every template on an eccentric orbit (one pair e cos w, e sin w != 0,
     so the template count is unchanged): the accumulation kernel's time against the circular search."""
     import dataclasses
-    wl = synth.config2()
+    wl = synth.widened(synth.config2(), 2)                   # 2 more margin bins: a_p Omega e f T < 1.2 bins at e = 0.03
     wle = dataclasses.replace(wl, ecosw=np.array([0.03 * math.cos(0.7)]), esinw=np.array([0.03 * math.sin(0.7)]))
-    out = {"workload": "config 2, every template with (e cos w, e sin w) = 0.03 (cos 0.7, sin 0.7)"}
+    out = {"workload": "config 2 on a slab with 2 more margin bins per side, every template with (e cos w, e sin w) = "
+                       "0.03 (cos 0.7, sin 0.7); same template count as the circular search"}
     for name, w in (("circular", wl), ("eccentric", wle)):
         patch = Patch(torch, bsh, ctx, w)
         for mode, mname in ((bsh.BSH_UNWEIGHTED, "unweighted"), (bsh.BSH_WEIGHTED, "weighted")):

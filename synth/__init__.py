@@ -394,6 +394,14 @@ def raw_sft_bins(seed: int, n_sft: int, n_raw: int, noise_sigma: float = 2.0) ->
     return np.ascontiguousarray(x * amp * np.sqrt(slope), np.complex64)
 
 
+def widened(wl: Workload, extra: int) -> Workload:
+    """The same workload on a slab with `extra` more margin columns on each side (fresh Exp(1) powers): room for the larger
+    excursion of eccentric tracks (a_p Omega e more bins), so that no track leaves the slab."""
+    n_bins = wl.n_bins + 2 * extra
+    return dataclasses.replace(wl, name=f"{wl.name}-wide{extra}", k_slab0=wl.k_slab0 - extra, n_bins=n_bins,
+                               rho=exp_powers(_rng(wl.seed, 5500 + extra), wl.n_sft, n_bins))
+
+
 def eccentric(wl: Workload, e_max: float = 0.05, n_e: int = 2, n_omega: int = 3) -> Workload:
     """The same workload with an eccentricity axis (Eq. 14, the ELL1 model for e << 1): pairs
     (e cos omega, e sin omega) on n_e rings e = e_max m / n_e (m = 1..n_e) x n_omega arguments of periapsis, plus the
