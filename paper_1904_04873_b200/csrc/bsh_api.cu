@@ -355,7 +355,8 @@ int dispatch_unweighted_pos(bsh_ctx *ctx, const Pending &pd, const PosParams &p,
 
 #define UNW_PIX_CASE(NW_, HP_, CL_)                                                                   \
     if (pd.NW == NW_ && pd.HP == HP_ && pd.clamp == CL_)                                              \
-        return launch_stage1(ctx, stage1_unweighted_pix_kernel<NW_, HP_, CL_>, p, 32 * kPixWarps, grid, pd.pix_smem);
+        return p.ke ? launch_stage1(ctx, stage1_unweighted_pix_kernel<NW_, HP_, CL_, true>, p, 32 * kPixWarps, grid, pd.pix_smem) \
+                    : launch_stage1(ctx, stage1_unweighted_pix_kernel<NW_, HP_, CL_, false>, p, 32 * kPixWarps, grid, pd.pix_smem);
 
 int dispatch_unweighted_pix(bsh_ctx *ctx, const Pending &pd, const PixParams &p, int grid)
 {
@@ -868,7 +869,8 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         const int stride = weighted ? PosStage<kWarpsWeighted, 1, true>(pg.n_pos).stride
                                     : PosStage<kWarpsUnweighted, 2, false>(pg.n_pos).stride;
         const int budgets[3] = {112 * 1024, 112 * 1024, 224 * 1024};                          // 2 / 2 / 1 blocks per SM
-        const int pix_budgets[3] = {113 * 1024, 113 * 1024, 224 * 1024};                      // (228 KB - 1 KB per block) / 2
+        const int pix_one = kPixWarps > 8 ? 224 * 1024 : 113 * 1024;                          // blocks of > 8 warps own an SM
+        const int pix_budgets[3] = {pix_one, pix_one, 224 * 1024};                            // (228 KB - 1 KB per block) / 2
         pd.n_stages = 0;
         for (int b = 0; b < 3 && pd.n_stages < 2; ++b) pd.n_stages = std::min(kMaxStages, (budgets[b] - kPosHeader) / stride);
         pd.use_pos = pd.n_stages >= 2 && fam != BSH_FAMILY_WINDOW && !(mode & BSH_NAIVE);

@@ -39,8 +39,12 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+#ifndef BSH_SPIN_DELAY
+#define BSH_SPIN_DELAY 0
+#endif
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 {
+#if BSH_SPIN_DELAY == 0
     asm volatile(
         "{\n\t"
         ".reg .pred P1;\n\t"
@@ -53,6 +57,20 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "}" ::"r"(smem_u32(bar)),
         "r"(parity)
         : "memory");
+#else
+    // a failed poll is followed by a chain of dependent MUFU operations (a pipe the accumulation kernels leave idle): the
+    // waiting warp then issues ~1 instruction per 20 cycles instead of spinning on the issue port the other warps need
+    uint32_t ok;
+    float x = 1.5f;
+    for (;;) {
+        asm volatile("{\n\t.reg .pred P1;\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\tselp.u32 %0, 1, 0, P1;\n\t}"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+        if (ok) break;
+#pragma unroll
+        for (int d = 0; d < BSH_SPIN_DELAY; ++d) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(x));
+        if (x == 123.456f) break;                         // never true: keeps the chain live
+    }
+#endif
 }
 __device__ __forceinline__ void tma_bulk_g2s(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *bar)
 {

@@ -26,7 +26,10 @@
 
 namespace bsh {
 
-constexpr int kPixWarps = 8;                         // warps per block
+#ifndef BSH_PIX_WARPS
+#define BSH_PIX_WARPS 8
+#endif
+constexpr int kPixWarps = BSH_PIX_WARPS;             // warps per block
 constexpr int kPixTpl = 2;                           // binary templates per thread
 constexpr int kPixTile = kPixWarps * kPixTpl;        // binary templates per block
 constexpr int kPixWarpScratch = kStageSfts * kPixTpl * 8 + kPixTpl * 32;       // B buffer of one stage + template constants
@@ -271,9 +274,11 @@ __device__ __forceinline__ void pix_half(const PixConst &k, uint32_t base, const
 }
 
 #ifndef BSH_PIX_MINB
-#define BSH_PIX_MINB 2
+#define BSH_PIX_MINB (BSH_PIX_WARPS > 8 ? 1 : 2)
 #endif
-template <int NW, int HP, bool CLAMP>
+// ECC: the grid has an eccentricity axis (Eq. 14); a template parameter, so that the circular search (Eq. 15) carries none of
+// its code (as a run-time branch it cost 2 % of the circular kernel's time)
+template <int NW, int HP, bool CLAMP, bool ECC>
 __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighted_pix_kernel(const PixParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -382,7 +387,7 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
             const double2 *cs = reinterpret_cast<const double2 *>(sp + L.tab_bytes);
             {   // binary terms of this stage: B = fl(A bracket)  (R-5, R-23), one per lane
                 const double2 c = cs[lane >> 1];
-                if (p.ke) {                              // eccentric grid (Eq. 14): the pair is re-read per stage (L1), so
+                if (ECC) {                     // eccentric grid (Eq. 14): the pair is re-read per stage (L1), so
                     const double2 ke_d = p.ke[rd ? it[1] : it[0]];   // that the circular search keeps its registers
                     bbuf[lane] = __dmul_rn(A_d, orbit_bracket(c.x, c.y, q_d.x, q_d.y, ke_d.x, ke_d.y));
                 } else {
@@ -421,7 +426,7 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
                 tc.u0 = kc.u0; tc.uL = kc.uL; tc.magic = kMagic; tc.off = p.off; tc.s_max = p.s_max; tc.s_zero = p.s_zero;
                 tc.n_fj = p.n_fj;
                 tc.A = tcst[r * 4 + 0]; tc.CA = tcst[r * 4 + 1]; tc.SA = tcst[r * 4 + 2];
-                const double2 ke_r = p.ke ? p.ke[it[r]] : make_double2(0.0, 0.0);
+                const double2 ke_r = ECC ? p.ke[it[r]] : make_double2(0.0, 0.0);
                 tc.kap = ke_r.x; tc.eta = ke_r.y;
                 uint32_t tp[kFixPlanes][NW];
 #pragma unroll

@@ -47,7 +47,8 @@ def test_library_is_built_for_sm_100a_with_tma_and_fp64_no_fma():
             assert "DMUL" in k and "DADD" in k and count_op in k, name
     pix = [k for k in kernels if k.startswith("_ZN3bsh28stage1_unweighted_pix_kernel")]
     assert all("LDS.64" in k for k in pix), "pixel-lane kernel: 8-byte window reads from the position-major table"
-    assert all("DSETP" in k for k in pix if "Lb0EEE" in k.split("\n")[0]), "unclamped pixel-lane kernel: FP64 break predicate"
+    assert all("DSETP" in k for k in pix if "Lb0ELb" in k.split("\n")[0]), "unclamped pixel-lane kernel: FP64 break predicate"
+    assert any("Lb0ELb0EEE" in k.split("\n")[0] for k in pix) and any("Lb0ELb1EEE" in k.split("\n")[0] for k in pix)
     wpix = [k for k in kernels if k.startswith("_ZN3bsh26stage1_weighted_pix_kernel")]
     assert all("R2P" in k for k in wpix), "weighted pixel-lane kernel: predicates of a byte of bins set by one R2P"
     front = [k for k in kernels if k.startswith("_ZN3bsh25normalise_peakgram_kernel")]
