@@ -35,7 +35,9 @@ namespace bsh {
 constexpr int kWpixWarps = BSH_WPIX_WARPS;           // warps (= binary templates) per block; one block per SM
 constexpr int kWpixHeader = 128 + kWpixWarps * kStageSfts * 8;   // mbarriers + one B buffer per warp
 
-// bins per byte-packed entry: NBYTES bytes of kWpixBits bins
+// BSH_WPIX_ROLL 1: one copy of the 16-SFT stage code serves both halves of a block of 32 (same speed as two copies, half the
+// code).  Rolling further (groups of 2 / 4 / 8 SFTs) measured 23.4 / 18.8 / 19.1 ms against 15.9 ms on config 2: the
+// look-ahead across the whole stage hides the load and FP64 latencies.
 #ifndef BSH_WPIX_ROLL
 #define BSH_WPIX_ROLL 1
 #endif
