@@ -25,7 +25,8 @@ P_PEAK = math.exp(-RHO_TH)                       # P(rho > r
 
 
 def build(force: bool = False) -> str:
-    """gcc -O2, no FMA contraction, OpenMP over templates."""
+    """gcc -O2, no FMA contraction, OpenMP over templates.  (Also builds the tier-2 reference.)"""
+    build_tier2(force)
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC", "-std=c11",
                "-Wall", "-o", _LIB, _SRC, "-lm"]
@@ -40,6 +41,37 @@ class _Problem(C.Structure):
                 ("n_ap", C.c_int32), ("ap", C.c_void_p), ("n_P", C.c_int32), ("P", C.c_void_p),
                 ("n_tasc", C.c_int32), ("tasc_frac", C.c_void_p),
                 ("n_ecc", C.c_int32), ("ecosw", C.c_void_p), ("esinw", C.c_void_p)]
+
+
+_SRC2 = os.path.join(_HERE, "bsh_tier2.c")
+_LIB2 = os.path.join(_HERE, "libbsh_tier2.so")
+_lib2 = None
+
+
+def build_tier2(force: bool = False) -> str:
+    """The tier-2 CPU reference (bsh_tier2.c): gcc -O3 (integer loops vectorise), no FMA contraction, OpenMP."""
+    if force or not os.path.exists(_LIB2) or os.path.getmtime(_LIB2) < os.path.getmtime(_SRC2):
+        cmd = ["gcc", "-O3", "-march=native", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
+               "-std=c11", "-Wall", "-o", _LIB2, _SRC2, "-lm"]
+        subprocess.run(cmd, check=True, capture_output=True)
+    return _LIB2
+
+
+def tier2_stage1(wl, peak: np.ndarray, w=None, n_threads=0, want_wcount=False):
+    """Tier-2 CPU reference (SURVEY 8(c) coverage plan): counts (and FP64 weighted counts) of EVERY template of the grid,
+    one track evaluation per (pixel, binary template, SFT).  Must equal stage1(..., mode=CANONICAL) bit for bit."""
+    global _lib2
+    if _lib2 is None:
+        _lib2 = C.CDLL(build_tier2())
+    pb = Problem(wl)
+    peak = np.ascontiguousarray(peak, np.uint32)
+    wv = None if w is None else np.ascontiguousarray(w, np.float32)
+    cnt = np.zeros(pb.n_templates, np.int32)
+    wc = np.zeros(pb.n_templates, np.float64) if want_wcount else None
+    _lib2.t2_stage1(pb.ref, C.c_void_p(peak.ctypes.data), C.c_int32(peak.shape[1]),
+                    C.c_void_p(wv.ctypes.data if wv is not None else None), C.c_void_p(cnt.ctypes.data),
+                    C.c_void_p(wc.ctypes.data if wc is not None else None), C.c_int(n_threads))
+    return (cnt, wc) if want_wcount else cnt
 
 
 _lib = None

@@ -342,6 +342,52 @@ def test_config2_full_size_unweighted(bsh, torch, ctx):
     check_toplist_complete(torch, torch.from_numpy(r["counts"]).cuda(), r["top"], wl.topk, weighted=False)
 
 
+def test_config2_full_grid_against_the_tier2_cpu_reference(bsh, torch, ctx):
+    """Every one of the 1.38e8 templates of config 2, both counts, against the tier-2 CPU reference (oracle/bsh_tier2.c),
+    which equals the plain oracle bit for bit wherever the plain oracle can run (tests/test_tier2.py): the chain
+    plain oracle == tier 2 == GPU of SURVEY.md 8(c)."""
+    wl = synth.config2()
+    pk = oracle.peakgram(wl.rho)
+    n_ref, w_ref = oracle.tier2_stage1(wl, pk, wl.w, want_wcount=True)
+    r = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=wl.topk)
+    assert np.array_equal(r["counts"], n_ref)
+    check_unweighted_toplist(r["top"], n_ref, wl.topk)
+    rw = gpu_stage1(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED, topk=wl.topk)
+    assert np.allclose(rw["counts"], w_ref, rtol=RTOL, atol=0)
+    check_float_toplist(rw["top"]["index"], w_ref, wl.topk)
+
+
+def test_config3_slice_config4_and_config5_patch_against_the_tier2_cpu_reference(bsh, torch, ctx):
+    """Full grids of a config-4 patch and a config-5 patch, and a 10 % slice (4 of the 40 a_p values) of the full-size
+    config-3 run, against the tier-2 CPU reference."""
+    # config 3: the GPU runs the FULL grid in the bench launch configuration; the slice of its dump is compared
+    wl = synth.config3()
+    pk = oracle.peakgram(wl.rho)
+    ia = [0, 13, 26, 39]
+    n_ref = oracle.tier2_stage1(wl.subgrid(ia=ia), pk)
+    d_rho, d_w = dev(torch, wl.rho), dev(torch, wl.w)
+    d_peak = ctx.build_peakgram(d_rho, 1.6)
+    d_counts = torch.full((wl.n_templates,), -7, dtype=torch.int32, device="cuda")
+    ctx.stage1_hough(d_peak, wl, mode=bsh.BSH_UNWEIGHTED, topk=wl.topk, d_w=d_w, counts_full=d_counts)
+    per_ap = len(wl.P) * len(wl.tasc_frac) * wl.n_f0
+    got = d_counts.view(wl.n_pix, len(wl.ap), per_ap)[:, ia, :].contiguous().view(-1).cpu().numpy()
+    assert np.array_equal(got, n_ref)
+    del d_counts
+    # config 4, patch 0 (with its injection), from |x|^2
+    c4 = synth.config4()
+    inj = c4.injections[0]
+    bins = [oracle.track(c4.patch_workload(i.patch, None), i.pix, i.ia, i.ip, i.it, i.j, mode=oracle.DIRECT) for i in c4.injections]
+    rho = c4.deposit(bins)
+    wl4 = c4.patch_workload(inj.patch, rho)
+    r = gpu_stage1(bsh, torch, ctx, wl4, bsh.BSH_UNWEIGHTED, topk=1000)
+    assert np.array_equal(r["counts"], oracle.tier2_stage1(wl4, oracle.peakgram(rho)))
+    # config 5, one patch at high declination
+    c5 = synth.config5()
+    wl5 = c5.patch_workload(15)
+    r = gpu_stage1(bsh, torch, ctx, wl5, bsh.BSH_UNWEIGHTED, topk=1000, rho=c5.base.rho)
+    assert np.array_equal(r["counts"], oracle.tier2_stage1(wl5, oracle.peakgram(c5.base.rho)))
+
+
 def test_config2_full_size_weighted(bsh, torch, ctx):
     _sampled_full_size_checks(bsh, torch, ctx, synth.config2(), weighted=True)
 
