@@ -37,7 +37,8 @@ extern "C" {
 #define BSH_ENOMEM   -2   /* device or host allocation failed                                                    */
 #define BSH_ECUDA    -3   /* a CUDA runtime call or kernel failed (message in bsh_last_error)                    */
 #define BSH_ESMALL   -4   /* an output buffer is too small (e.g. words_per_row * 32 < n_bins)                    */
-#define BSH_ESTATE   -5   /* call order violated (e.g. bsh_stage1_collect without bsh_stage1_launch)             */
+#define BSH_ESTATE   -5   /* call order violated (e.g. bsh_stage1_collect without bsh_stage1_launch), or the candidate  */
+                          /* selection did not converge (degenerate input); message in bsh_last_error              */
 
 /* mode bits for stage 1 */
 #define BSH_UNWEIGHTED 0  /* rank by the integer number count n                                   (L223)         */
@@ -107,7 +108,8 @@ typedef struct {
     int64_t  n_candidates;       /* templates that passed the in-kernel threshold                                  */
     double   threshold;          /* final in-kernel threshold (count or weighted count)                            */
     int32_t  n_passes;           /* accumulation passes (1 unless the threshold had to be moved)                   */
-    int32_t  kernel_variant;     /* words * 100 + pixels_per_thread * 10 + clamp                                   */
+    int32_t  kernel_variant;     /* family * 1000 + words * 100 + pixels_per_thread * 10 + clamp; family 3 = weighted  */
+                                 /* pixel-lane, 2 = pixel-lane, 1 = template-lane position table, 0 = funnel-shift     */
     int32_t  threads_per_block;  /* of the accumulation kernel                                                     */
     int32_t  grid_blocks;        /* of the accumulation kernel                                                     */
     int64_t  launches;           /* kernels launched by this context since creation                                */
@@ -171,7 +173,7 @@ double bsh_median_bias(int32_t window);    /* sum_{i = (window + 1) / 2}^{window
  * peakgram, and the per-patch toplist (L217, L225).
  *   d_peak          [n_sft][words_per_row] as written by bsh_build_peakgram for this SFT set
  *   mode            BSH_UNWEIGHTED or BSH_WEIGHTED (needs sfts->d_w), optionally | BSH_NAIVE
- *   topk            entries wanted, 1 <= topk
+ *   topk            entries wanted, 1 <= topk <= 2^27 (BSH_EINVAL beyond the candidate buffer)
  *   d_top           [topk] records, best first; entries beyond *h_n_top are zeroed
  *   h_n_top         receives min(topk, n_templates)
  *   d_counts_full   optional dump of the ranking statistic of EVERY template (int32 counts in BSH_UNWEIGHTED mode,
@@ -181,7 +183,10 @@ double bsh_median_bias(int32_t window);    /* sum_{i = (window + 1) / 2}^{window
  * bsh_stage1_launch is asynchronous (no host synchronisation); bsh_stage1_collect synchronises the stream, runs the
  * selection, and leaves the toplist writes enqueued on the stream (h_n_top is final on return).  Between launch and
  * collect the caller may enqueue work on OTHER contexts/streams (this is how config 5 overlaps two patches).
- * The host arrays inside `sfts` and `grid` are read during launch only. */
+ * The host arrays inside `sfts` and `grid` are read during launch only; the DEVICE buffers d_peak, sfts->d_w and
+ * d_counts_full are read / written until bsh_stage1_collect returns (toplist rescoring and threshold retries) and must stay
+ * valid until then.  Other calls on the same context between launch and collect are allowed (their tables use the other
+ * cache slot). */
 int bsh_stage1_hough(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_row, const bsh_sfts *sfts,
                      const bsh_grid *grid, int32_t mode, int32_t topk, bsh_cand *d_top, int32_t *h_n_top,
                      void *d_counts_full);
@@ -190,7 +195,8 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
 int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top);
 
 /* Stage 2 (Eq. 26): power[c] = sum_i w_i rho[i][k_i] along the track of d_cands[c].index over the SFT set
- * `sfts` (FP32 products, each lane sums every 32nd SFT in order, then a fixed shuffle tree; R-20), written into
+ * `sfts` (FP32 products; thread t of the candidate's 128-thread block sums SFTs t, t + 128, ... in order, then a fixed shuffle
+ * tree per warp and the warp partials in warp order; R-20), written into
  * d_cands[c].power.  If sort_by_power != 0 the records are then reordered by (power desc, index asc).
  * d_rho: [n_sft][rho_row_stride] FP32.  Asynchronous. */
 int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, const bsh_sfts *sfts,

@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbsh.so")
 SOURCES = [os.path.join(CSRC, "bsh_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "bsh_kernels.cuh"), os.path.join(CSRC, "bsh_core.cuh"),
-                  os.path.join(CSRC, "bsh_pos.cuh"), os.path.join(CSRC, "bsh_pix.cuh"), os.path.join(CSRC, "bsh_peaks.cuh"), os.path.join(CSRC, "bsh_wpix.cuh"), os.path.join(CSRC, "bsh_frontend.cuh"), os.path.join(CSRC, "bsh_post.cuh"),
+                  os.path.join(CSRC, "bsh_pos.cuh"), os.path.join(CSRC, "bsh_pix.cuh"), os.path.join(CSRC, "bsh_peaks.cuh"), os.path.join(CSRC, "bsh_wpix.cuh"), os.path.join(CSRC, "bsh_frontend.cuh"), os.path.join(CSRC, "bsh_post.cuh"), os.path.join(CSRC, "bsh_sort.cuh"),
                   os.path.join(CSRC, "bsh_host.hpp"),
                   os.path.join(HERE, "..", "include", "bsh.h")]
 

@@ -21,6 +21,7 @@
 #include "bsh_peaks.cuh"
 #include "bsh_frontend.cuh"
 #include "bsh_post.cuh"
+#include "bsh_sort.cuh"
 
 using namespace bsh;
 
@@ -40,7 +41,8 @@ struct TableCache {                   // cos/sin tables of one (SFT set, binary 
     std::vector<double> t_mid, v, P, tasc, ap, ecw, esw;
     double t_sft = 0, t_search_mid = 0;
     int n_sft = 0, n_pad = 0, n_P = 0, n_tasc = 0, n_ap = 0, n_ecc = 0;
-    DevBuf d_v, d_cs, d_casa, d_A, d_ke;
+    DevBuf d_v, d_cs, d_casa, d_A, d_ke, d_cs_t;
+    bool have_cs_t = false;
 };
 
 struct Pending {                      // state between bsh_stage1_launch and bsh_stage1_collect
@@ -87,6 +89,7 @@ struct bsh_ctx {
     int opt_family = BSH_FAMILY_AUTO, opt_force_clamp = 0, opt_pixels_per_thread = 0;   // bsh_set_option
     DevBuf peak_samples;
     DevBuf post_adj, post_cnt, post_off, post_tmp;
+    DevBuf radix_hist;
     bsh_stats st = {};
     bool have_front = false;
     bool have_pk = false, have_setup = false, have_kernel = false, have_select = false, have_s2 = false;
@@ -223,6 +226,7 @@ int get_tables(bsh_ctx *ctx, const bsh_sfts *s, const bsh_grid *g, int *slot_out
     if (ctx->pend.active && ctx->pend.cache_slot == k) k ^= 1;     // a launched, uncollected stage 1 still reads its slot
     TableCache &c = ctx->cache[k];
     c.valid = false;
+    c.have_cs_t = false;
     const int n_pad = pad_sfts(N);
     c.t_mid.assign(s->h_t_mid, s->h_t_mid + N);
     c.v.assign(s->h_v_over_c, s->h_v_over_c + 3 * (size_t)N);
@@ -274,6 +278,20 @@ int build_dtable(bsh_ctx *ctx, const bsh_grid *g, const TableCache &c, int R, De
     return BSH_OK;
 }
 
+// transposed (cos, sin) table of a cache slot, built on first use by the large-list kernels
+int ensure_cs_t(bsh_ctx *ctx, TableCache &c)
+{
+    if (c.have_cs_t) return BSH_OK;
+    const int64_t n = (int64_t)c.n_P * c.n_pad;
+    TRY(ensure(ctx, c.d_cs_t, sizeof(double) * 2 * (size_t)n));
+    transpose_cs_kernel<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>((const double2 *)c.d_cs.p, c.n_P, c.n_pad,
+                                                                            (double2 *)c.d_cs_t.p);
+    count_launch(ctx);
+    CK(cudaGetLastError());
+    c.have_cs_t = true;
+    return BSH_OK;
+}
+
 TrackTables make_track_tables(const TableCache &c, const bsh_sfts *s, const bsh_grid *g, const double *dtab, int R)
 {
     TrackTables t;
@@ -282,6 +300,7 @@ TrackTables make_track_tables(const TableCache &c, const bsh_sfts *s, const bsh_
     t.A = (const double *)c.d_A.p;
     t.casa = (const double2 *)c.d_casa.p;
     t.ke = c.n_ecc > 0 ? (const double2 *)c.d_ke.p : nullptr;
+    t.cs_t = nullptr;
     t.n_pad = c.n_pad;
     t.R = R;
     t.n_pix = g->n_pix; t.n_ap = g->n_ap; t.n_P = g->n_P; t.n_tasc = g->n_tasc; t.n_f0 = g->n_f0;
@@ -578,6 +597,40 @@ int sort_candidates(bsh_ctx *ctx, RawCand *buf, unsigned int n)
     return BSH_OK;
 }
 
+constexpr unsigned int kRadixMin = 1u << 16;      // above this many records the radix sort replaces the bitonic network
+
+// Large lists: stable LSD radix sort by (key desc, index asc), one pass per byte of the composite key in
+// which the records differ.  buf and tmp hold n records each; *out = the buffer that ends up sorted.  Synchronises once.
+int radix_sort_candidates(bsh_ctx *ctx, RawCand *buf, RawCand *tmp, unsigned int n, RawCand **out)
+{
+    *out = buf;
+    if (n <= 1) return BSH_OK;
+    const unsigned int n_tiles = (n + kRadixTile - 1) / kRadixTile;
+    TRY(ensure(ctx, ctx->radix_hist, 64 + (size_t)256 * n_tiles * 4));
+    unsigned int *d_diff = (unsigned int *)ctx->radix_hist.p;
+    unsigned int *d_hist = d_diff + 16;
+    CK(cudaMemsetAsync(d_diff, 0, 12, ctx->stream));
+    radix_diff_kernel<<<std::min(1024u, (n + 255) / 256), 256, 0, ctx->stream>>>(buf, n, d_diff);
+    count_launch(ctx);
+    CK(cudaMemcpyAsync(ctx->pinned_count + 10, d_diff, 12, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    const uint64_t di = (uint64_t)ctx->pinned_count[10] | ((uint64_t)ctx->pinned_count[11] << 32);
+    const uint32_t dk = ctx->pinned_count[12];
+    RawCand *src = buf, *dst = tmp;
+    for (int pass = 0; pass < 12; ++pass) {
+        const bool varies = pass < 8 ? ((di >> (8 * pass)) & 255u) != 0 : ((dk >> (8 * (pass - 8))) & 255u) != 0;
+        if (!varies) continue;
+        radix_hist_kernel<<<n_tiles, kRadixThreads, 0, ctx->stream>>>(src, n, pass, n_tiles, d_hist);
+        radix_scan_kernel<<<1, 1024, 0, ctx->stream>>>(d_hist, 256u * n_tiles);
+        radix_scatter_kernel<<<n_tiles, kRadixThreads, 0, ctx->stream>>>(src, n, pass, n_tiles, d_hist, dst);
+        count_launch(ctx, 3);
+        std::swap(src, dst);
+    }
+    CK(cudaGetLastError());
+    *out = src;
+    return BSH_OK;
+}
+
 }  // namespace
 
 namespace {
@@ -640,11 +693,11 @@ int bsh_destroy(bsh_ctx *ctx)
     cudaStreamSynchronize(ctx->stream);
     DevBuf *bufs[] = {&ctx->wtab, &ctx->w_pad, &ctx->stats, &ctx->thr, &ctx->dtab, &ctx->nvec, &ctx->cand, &ctx->cand_count,
                       &ctx->keys, &ctx->tmp_cands, &ctx->dtab2, &ctx->nvec2, &ctx->ptab, &ctx->dpos, &ctx->dpix, &ctx->psplit, &ctx->tab7, &ctx->h_rho, &ctx->h_w, &ctx->h_peak, &ctx->h_top, &ctx->peak_samples,
-                      &ctx->post_adj, &ctx->post_cnt, &ctx->post_off, &ctx->post_tmp};
+                      &ctx->post_adj, &ctx->post_cnt, &ctx->post_off, &ctx->post_tmp, &ctx->radix_hist};
     for (DevBuf *b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto &c : ctx->cache) {
-        DevBuf *cb[] = {&c.d_v, &c.d_cs, &c.d_casa, &c.d_A, &c.d_ke};
+        DevBuf *cb[] = {&c.d_v, &c.d_cs, &c.d_casa, &c.d_A, &c.d_ke, &c.d_cs_t};
         for (DevBuf *b : cb)
             if (b->p) cudaFree(b->p);
     }
@@ -896,6 +949,8 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
         const uint64_t need = std::min<uint64_t>(pd.n_templates, 4ull * (uint64_t)topk);
         while (pd.cand_cap < need && pd.cand_cap < (1u << 27)) pd.cand_cap <<= 1;
     }
+    if (std::min<uint64_t>((uint64_t)topk, pd.n_templates) > pd.cand_cap)
+        return fail(ctx, BSH_EINVAL, "topk = %d exceeds the candidate buffer (%u entries)", topk, pd.cand_cap);
     pd.emit_all = pd.n_templates <= pd.cand_cap;
     pd.frac = (double)std::max<int64_t>(8ll * topk, 4096) / (double)pd.n_templates;
     if ((uint64_t)topk > kCandCap / 8) pd.frac = (1.3 * (double)topk + 4096.0) / (double)pd.n_templates;
@@ -1005,12 +1060,14 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
         n_cand = ctx->pinned_count[0];
         const bool too_few = n_cand < want, too_many = n_cand > pd.cand_cap;
         if (!too_few && !too_many) break;
-        if (pd.passes >= kMaxPasses) return fail(ctx, BSH_ECUDA, "candidate selection did not converge (%u candidates)", n_cand);
+        if (pd.passes >= kMaxPasses)
+            return fail(ctx, BSH_ESTATE, "candidate selection did not converge after %d passes (%u candidates for topk %d; degenerate "
+                                         "input: constant rows or massive ties at the cut?)", pd.passes, n_cand, pd.topk);
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, ctx->ev[2], ctx->ev[3]) == cudaSuccess) ctx->kernel_ms_extra += ms;
         if (too_few) {
             pd.shift_sigma -= 0.75;
-            if (pd.passes >= 6) { pd.emit_all = true; }
+            if (pd.passes >= 6 && pd.n_templates <= pd.cand_cap) pd.emit_all = true;   // (else emit_all would overflow the buffer)
         } else {
             pd.emit_all = false;
             pd.shift_sigma += 0.5;
@@ -1027,7 +1084,10 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
 
     CK(cudaEventRecord(ctx->ev[4], ctx->stream));
     RawCand *sorted = (RawCand *)ctx->cand.p;
-    if (n_cand > (unsigned)kSortTile && (uint64_t)n_cand > want) {
+    if (n_cand > kRadixMin) {
+        TRY(ensure(ctx, ctx->keys, (size_t)pd.cand_cap * sizeof(RawCand)));
+        TRY(radix_sort_candidates(ctx, (RawCand *)ctx->cand.p, (RawCand *)ctx->keys.p, n_cand, &sorted));
+    } else if (n_cand > (unsigned)kSortTile && (uint64_t)n_cand > want) {
         // only the candidates at or above the k-th largest key take part in the sort (ties at the cut included)
         TRY(ensure(ctx, ctx->keys, (size_t)pd.cand_cap * sizeof(RawCand)));
         select_cut_kernel<<<1, 1024, 0, ctx->stream>>>((const RawCand *)ctx->cand.p, n_cand, (unsigned int)want,
@@ -1052,9 +1112,19 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
         s.n_sft = pd.n_sft; s.k_slab0 = pd.k_slab0; s.n_bins = pd.n_bins;
         bsh_grid g = {};
         g.n_pix = pd.n_pix; g.n_ap = pd.n_ap; g.n_P = pd.n_P; g.n_tasc = pd.n_tasc; g.n_f0 = pd.n_f0; g.k_band0 = pd.k_band0;
-        const TrackTables t = make_track_tables(c, &s, &g, (const double *)ctx->dtab.p, pd.R);
-        rescore_kernel<<<n_keep, kCandThreads, 0, ctx->stream>>>(t, pd.d_peak, pd.words_per_row, pd.d_w,
-                                                                          weighted ? 1 : 0, d_top, n_keep);
+        TrackTables t = make_track_tables(c, &s, &g, (const double *)ctx->dtab.p, pd.R);
+        if ((unsigned)n_keep > kRadixMin) {
+            TRY(ensure_cs_t(ctx, ctx->cache[pd.cache_slot]));
+            t.cs_t = (const double2 *)c.d_cs_t.p;
+            if (t.ke)
+                rescore_rows_kernel<true><<<(n_keep + 255) / 256, 256, 0, ctx->stream>>>(t, pd.d_peak, pd.words_per_row, pd.d_w,
+                                                                                         weighted ? 1 : 0, d_top, n_keep);
+            else
+                rescore_rows_kernel<false><<<(n_keep + 255) / 256, 256, 0, ctx->stream>>>(t, pd.d_peak, pd.words_per_row, pd.d_w,
+                                                                                          weighted ? 1 : 0, d_top, n_keep);
+        } else
+            rescore_kernel<<<n_keep, kCandThreads, 0, ctx->stream>>>(t, pd.d_peak, pd.words_per_row, pd.d_w,
+                                                                              weighted ? 1 : 0, d_top, n_keep);
         count_launch(ctx);
     }
     CK(cudaGetLastError());
@@ -1090,25 +1160,38 @@ int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, c
     TRY(get_tables(ctx, sfts, grid, &slot));
     const TableCache &c = ctx->cache[slot];
     CK(cudaEventRecord(ctx->ev[6], ctx->stream));
-    TRY(build_dtable(ctx, grid, c, 1, ctx->nvec2, ctx->dtab2));
+    const bool rows = (unsigned)n_cands > kRadixMin;       // large lists: D laid out [SFT][pixel], (cos, sin) transposed
+    const int R2 = rows ? grid->n_pix : 1;
+    TRY(build_dtable(ctx, grid, c, R2, ctx->nvec2, ctx->dtab2));
     const bsh_grid kg = kernel_grid(grid);
-    const TrackTables t = make_track_tables(c, sfts, &kg, (const double *)ctx->dtab2.p, 1);
-    stage2_kernel<<<(unsigned)n_cands, kCandThreads, 0, ctx->stream>>>(t, d_rho, rho_row_stride,
-                                                                                          sfts->d_w, d_cands, n_cands);
+    TrackTables t = make_track_tables(c, sfts, &kg, (const double *)ctx->dtab2.p, R2);
+    if (rows) {
+        TRY(ensure_cs_t(ctx, ctx->cache[slot]));
+        t.cs_t = (const double2 *)c.d_cs_t.p;
+    }
+    if (rows && t.ke)
+        stage2_rows_kernel<true><<<(n_cands + 255) / 256, 256, 0, ctx->stream>>>(t, d_rho, rho_row_stride, sfts->d_w, d_cands, n_cands);
+    else if (rows)
+        stage2_rows_kernel<false><<<(n_cands + 255) / 256, 256, 0, ctx->stream>>>(t, d_rho, rho_row_stride, sfts->d_w, d_cands, n_cands);
+    else
+        stage2_kernel<<<(unsigned)n_cands, kCandThreads, 0, ctx->stream>>>(t, d_rho, rho_row_stride, sfts->d_w, d_cands, n_cands);
     count_launch(ctx);
     CK(cudaGetLastError());
     if (sort_by_power && n_cands > 1) {
         unsigned int n2 = 1;
         while (n2 < (unsigned)n_cands) n2 <<= 1;
-        TRY(ensure(ctx, ctx->keys, (size_t)n2 * sizeof(RawCand)));
+        const bool large = (unsigned)n_cands > kRadixMin;
+        TRY(ensure(ctx, ctx->keys, (size_t)n2 * sizeof(RawCand) * (large ? 2 : 1)));
         TRY(ensure(ctx, ctx->tmp_cands, (size_t)n_cands * sizeof(bsh_cand)));
         pack_power_keys_kernel<<<(n_cands + 255) / 256, 256, 0, ctx->stream>>>(d_cands, n_cands, (RawCand *)ctx->keys.p);
         count_launch(ctx);
-        TRY(sort_candidates(ctx, (RawCand *)ctx->keys.p, (unsigned)n_cands));
+        RawCand *order = (RawCand *)ctx->keys.p;
+        if (large) TRY(radix_sort_candidates(ctx, (RawCand *)ctx->keys.p, (RawCand *)ctx->keys.p + n2, (unsigned)n_cands, &order));
+        else TRY(sort_candidates(ctx, (RawCand *)ctx->keys.p, (unsigned)n_cands));
         CK(cudaMemcpyAsync(ctx->tmp_cands.p, d_cands, (size_t)n_cands * sizeof(bsh_cand), cudaMemcpyDeviceToDevice,
                            ctx->stream));
         permute_cands_kernel<<<(n_cands + 255) / 256, 256, 0, ctx->stream>>>((const bsh_cand *)ctx->tmp_cands.p,
-                                                                            (const RawCand *)ctx->keys.p, n_cands, d_cands);
+                                                                            (const RawCand *)order, n_cands, d_cands);
         count_launch(ctx);
         CK(cudaGetLastError());
     }

@@ -62,12 +62,8 @@ BSH_HD int32_t round_int(double y)
 #endif
 }
 
-// s = off + round(fl(u g))   (`magic` is unused: kept so that the call sites read as before)
-BSH_HD int32_t shift_of(double u, double g, double magic, int32_t off)
-{
-    (void)magic;
-    return off + round_int(dmul(u, g));
-}
+// s = off + round(fl(u g))
+BSH_HD int32_t shift_of(double u, double g, int32_t off) { return off + round_int(dmul(u, g)); }
 
 BSH_HD uint32_t funnel_r(uint32_t lo, uint32_t hi, int sh)   // low 32 bits of ((hi:lo) >> (sh & 31))
 {
@@ -164,7 +160,7 @@ BSH_HD_NOINLINE Win<NW> break_window(const uint4 *row_entries, double g, double 
         int lo = 0, hi = n_fj - 1;                       // shift(lo) == s0, shift(hi) == sL
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
-            const int32_t sm = shift_of(dadd(u0, (double)mid), g, magic, off);
+            const int32_t sm = shift_of(dadd(u0, (double)mid), g, off);
             if (sm == s0) lo = mid; else hi = mid;
         }
         const Win<NW> a = load_window<NW>(row_entries, CLAMP ? clamp_s(s0, s_max) : s0);
@@ -180,7 +176,7 @@ BSH_HD_NOINLINE Win<NW> break_window(const uint4 *row_entries, double g, double 
 #pragma unroll
     for (int w = 0; w < NW; ++w) out.x[w] = 0u;
     for (int j = 0; j < n_fj; ++j) {
-        const int32_t sj = shift_of(dadd(u0, (double)j), g, magic, off);
+        const int32_t sj = shift_of(dadd(u0, (double)j), g, off);
         const uint32_t bit = table_bit(row_entries, sj + j, s_max >> 5);
 #pragma unroll
         for (int w = 0; w < NW; ++w)
@@ -194,8 +190,8 @@ template <int NW, bool CLAMP>
 BSH_HD Win<NW> track_window(const TrackConst &tc, const uint4 *row_entries, double D, double B)
 {
     const double g = dsub(D, B);
-    const int32_t s0 = shift_of(tc.u0, g, tc.magic, tc.off);
-    const int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
+    const int32_t s0 = shift_of(tc.u0, g, tc.off);
+    const int32_t sL = shift_of(tc.uL, g, tc.off);
     if (s0 != sL) return break_window<NW, CLAMP>(row_entries, g, tc.u0, tc.magic, tc.off, tc.n_fj, tc.s_max, s0, sL);
     return load_window<NW>(row_entries, CLAMP ? clamp_s(s0, tc.s_max) : s0);
 }
@@ -208,8 +204,8 @@ template <int NW, bool CLAMP>
 BSH_HD Win<NW> track_window_deferred(const TrackConst &tc, const uint4 *row_entries, double D, double B, bool &brk)
 {
     const double g = dsub(D, B);
-    const int32_t s0 = shift_of(tc.u0, g, tc.magic, tc.off);
-    const int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
+    const int32_t s0 = shift_of(tc.u0, g, tc.off);
+    const int32_t sL = shift_of(tc.uL, g, tc.off);
     brk = s0 != sL;
     int32_t s = CLAMP ? clamp_s(s0, tc.s_max) : s0;
     s = brk ? tc.s_zero : s;
@@ -266,7 +262,7 @@ BSH_HD_NOINLINE Win<NW> break_window_pos(const uint4 *row_positions, double g, d
         int lo = 0, hi = n_fj - 1;                       // shift(lo) == s0, shift(hi) == sL
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
-            const int32_t sm = shift_of(dadd(u0, (double)mid), g, magic, off);
+            const int32_t sm = shift_of(dadd(u0, (double)mid), g, off);
             if (sm == s0) lo = mid; else hi = mid;
         }
         const Win<NW> a = load_position<NW>(row_positions, CLAMP ? clamp_s(s0, s_max) : s0);
@@ -282,7 +278,7 @@ BSH_HD_NOINLINE Win<NW> break_window_pos(const uint4 *row_positions, double g, d
 #pragma unroll
     for (int w = 0; w < NW; ++w) out.x[w] = 0u;
     for (int j = 0; j < n_fj; ++j) {
-        int32_t sj = shift_of(dadd(u0, (double)j), g, magic, off);
+        int32_t sj = shift_of(dadd(u0, (double)j), g, off);
         sj = clamp_s(sj, s_max);                         // in the unclamped geometry this is the identity (proven range)
         const uint4 e = row_positions[sj];
         const uint32_t word = (j >> 5) == 0 ? e.x : ((j >> 5) == 1 ? e.y : e.z);
@@ -298,8 +294,8 @@ template <int NW, bool CLAMP>
 BSH_HD Win<NW> track_window_pos(const TrackConst &tc, const uint4 *row_positions, double D, double B)
 {
     const double g = dsub(D, B);
-    const int32_t s0 = shift_of(tc.u0, g, tc.magic, tc.off);
-    const int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
+    const int32_t s0 = shift_of(tc.u0, g, tc.off);
+    const int32_t sL = shift_of(tc.uL, g, tc.off);
     if (s0 != sL) return break_window_pos<NW, CLAMP>(row_positions, g, tc.u0, tc.magic, tc.off, tc.n_fj, tc.s_max, s0, sL);
     return load_position<NW>(row_positions, CLAMP ? clamp_s(s0, tc.s_max) : s0);
 }
@@ -309,8 +305,8 @@ template <bool CLAMP>
 BSH_HD int32_t track_position_deferred(const TrackConst &tc, double D, double B, bool &brk)
 {
     const double g = dsub(D, B);
-    int32_t s0 = shift_of(tc.u0, g, tc.magic, tc.off);
-    int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
+    int32_t s0 = shift_of(tc.u0, g, tc.off);
+    int32_t sL = shift_of(tc.uL, g, tc.off);
     if (CLAMP) { s0 = clamp_s(s0, tc.s_max); sL = clamp_s(sL, tc.s_max); }   // equal after clamping => every bin reads 0
     brk = s0 != sL;
     return brk ? tc.s_zero : s0;
@@ -476,14 +472,14 @@ BSH_HD Win<NW> exact_window_pos(const TrackConst &tc, const uint4 *row_positions
     const double y0 = dmul(tc.u0, g);
     const int32_t r0 = round_int(y0);
     const int32_t s0 = tc.off + r0;
-    const int32_t sL = shift_of(tc.uL, g, tc.magic, tc.off);
+    const int32_t sL = shift_of(tc.uL, g, tc.off);
     const int32_t d = sL - s0;
     if (CLAMP || (d != 1 && d != -1)) return track_window_pos<NW, CLAMP>(tc, row_positions, D, B);
     const float dist = (float)(((double)r0 + (d > 0 ? 0.5 : -0.5)) - y0);     // signed distance to the crossed half-integer
     int j = (int)ceilf(fast_divide(dist, (float)g));
     j = j < 1 ? 1 : (j > tc.n_fj - 1 ? tc.n_fj - 1 : j);
-    while (j > 1 && shift_of(dadd(tc.u0, (double)(j - 1)), g, tc.magic, tc.off) != s0) --j;
-    while (j < tc.n_fj - 1 && shift_of(dadd(tc.u0, (double)j), g, tc.magic, tc.off) == s0) ++j;
+    while (j > 1 && shift_of(dadd(tc.u0, (double)(j - 1)), g, tc.off) != s0) --j;
+    while (j < tc.n_fj - 1 && shift_of(dadd(tc.u0, (double)j), g, tc.off) == s0) ++j;
     const Win<NW> a = load_position<NW>(row_positions, s0);
     const Win<NW> b = load_position<NW>(row_positions, sL);
     Win<NW> out;

@@ -542,6 +542,7 @@ struct TrackTables {
     const double *A;       // [n_ap][n_P]
     const double2 *casa;   // [n_P][n_tasc]
     const double2 *ke;     // [n_tasc] (e cos omega, e sin omega), or NULL (circular orbits)
+    const double2 *cs_t;   // [n_pad][n_P] transposed copy of cs for the one-thread-per-candidate kernels, or NULL
     int n_pad, R;
     int n_pix, n_ap, n_P, n_tasc, n_f0;
     int64_t k_band0;
@@ -565,7 +566,7 @@ struct TemplateConst {
     double A, CA, SA, u, kap, eta;
     const double2 *cs;
     const double *d;
-    int d_stride, mj;
+    int d_stride, cs_stride, mj;
 };
 
 __device__ __forceinline__ TemplateConst template_const(const TrackTables &t, const TemplateCoord &c)
@@ -579,19 +580,24 @@ __device__ __forceinline__ TemplateConst template_const(const TrackTables &t, co
     k.kap = ke.x;
     k.eta = ke.y;
     k.u = (double)(t.k_band0 + c.j);
-    k.cs = t.cs + (int64_t)c.ip * t.n_pad;
+    k.cs = t.cs_t ? t.cs_t + c.ip : t.cs + (int64_t)c.ip * t.n_pad;
+    k.cs_stride = t.cs_t ? t.n_P : 1;
     k.d = t.dtab + ((int64_t)(c.pix / t.R) * t.n_pad) * t.R + (c.pix % t.R);
     k.d_stride = t.R;
     k.mj = t.m + c.j;
     return k;
 }
 
+// ECC = false: the grid is circular (Eq. 15), the eccentric terms are not even compiled in (as a run-time test of kap, eta the
+// compiler evaluated both brackets and selected: 19 instead of 9 FP64 operations per evaluation in the large-list kernels)
+template <bool ECC = true>
 __device__ __forceinline__ int track_column(const TemplateConst &k, int i, int n_bins)
 {
-    const double2 cs = k.cs[i];
-    const double B = dmul(k.A, orbit_bracket(cs.x, cs.y, k.CA, k.SA, k.kap, k.eta));
+    const double2 cs = k.cs[(int64_t)i * k.cs_stride];
+    const double B = dmul(k.A, ECC ? orbit_bracket(cs.x, cs.y, k.CA, k.SA, k.kap, k.eta)
+                                   : dadd(dmul(cs.x, k.CA), dmul(cs.y, k.SA)));
     const double g = dsub(k.d[(int64_t)i * k.d_stride], B);
-    const int col = shift_of(k.u, g, kMagic + (double)k.mj, k.mj);
+    const int col = shift_of(k.u, g, k.mj);
     return (col >= 0 && col < n_bins) ? col : -1;
 }
 
@@ -874,6 +880,77 @@ __global__ void __launch_bounds__(kCandThreads) stage2_kernel(const TrackTables 
         cands[c].power = pw;
         cands[c].flags |= 2u;
     }
+}
+
+// LARGE candidate lists (a fraction N_C of the bank, millions of candidates): one THREAD per candidate, the block's
+// 256 candidates walk the SFTs together, so that row i of the power slab (or of the peakgram), D[.][i] and (cos, sin)[.][i]
+// are fetched once per block and served to its threads by L1 -- with one block per candidate every gather pulls its own
+// 32-byte sector through L2 (measured 2.4e11 gathers/s).  FP32 sums (R-20): partial sums over chunks of kRowChunk SFTs in
+// SFT order, then the partials in chunk order.
+constexpr int kRowChunk = 128;
+
+// cs_t[i][p] = cs[p][i]: with the periods of one SFT contiguous (and D laid out [SFT][pixel]: dtable_kernel with R = n_pix),
+// the table reads of a warp whose lanes hold different templates fall into a few cache lines per SFT instead of one each
+__global__ void __launch_bounds__(256) transpose_cs_kernel(const double2 *__restrict__ cs, int n_P, int n_pad,
+                                                           double2 *__restrict__ cs_t)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (int64_t)n_P * n_pad) return;
+    const int i = (int)(t / n_P), p = (int)(t % n_P);
+    cs_t[t] = cs[(int64_t)p * n_pad + i];
+}
+
+template <bool ECC>
+__global__ void __launch_bounds__(256) stage2_rows_kernel(const TrackTables t, const float *__restrict__ rho, int64_t stride,
+                                                          const float *__restrict__ w, bsh_cand *__restrict__ cands, int n_cands)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n_cands) return;
+    const TemplateCoord tc = decode_template(t, cands[c].index);
+    const TemplateConst k = template_const(t, tc);
+    float total = 0.0f;
+    for (int i0 = 0; i0 < t.n_sft; i0 += kRowChunk) {
+        const int i1 = i0 + kRowChunk < t.n_sft ? i0 + kRowChunk : t.n_sft;
+        float part = 0.0f;
+#pragma unroll 8
+        for (int i = i0; i < i1; ++i) {                   // (unrolled: the loads of 8 SFTs are in flight together)
+            const int col = track_column<ECC>(k, i, t.n_bins);
+            const float r = __ldg(rho + (int64_t)i * stride + (col >= 0 ? col : 0));
+            if (col >= 0) part += (w ? __ldg(w + i) : 1.0f) * r;
+        }
+        total += part;
+    }
+    cands[c].power = total;
+    cands[c].flags |= 2u;
+}
+
+template <bool ECC>
+__global__ void __launch_bounds__(256) rescore_rows_kernel(const TrackTables t, const uint32_t *__restrict__ peak,
+                                                           int words_per_row, const float *__restrict__ w, int weighted_rank,
+                                                           bsh_cand *__restrict__ cands, int n_cands)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n_cands) return;
+    const TemplateCoord tc = decode_template(t, cands[c].index);
+    const TemplateConst k = template_const(t, tc);
+    int n = 0;
+    float total = 0.0f;
+    for (int i0 = 0; i0 < t.n_sft; i0 += kRowChunk) {
+        const int i1 = i0 + kRowChunk < t.n_sft ? i0 + kRowChunk : t.n_sft;
+        float part = 0.0f;
+#pragma unroll 8
+        for (int i = i0; i < i1; ++i) {
+            const int col = track_column<ECC>(k, i, t.n_bins);
+            const uint32_t word = __ldg(peak + (int64_t)i * words_per_row + ((col >= 0 ? col : 0) >> 5));
+            if (col >= 0 && ((word >> (col & 31)) & 1u)) {
+                n += 1;
+                part += w ? __ldg(w + i) : 1.0f;
+            }
+        }
+        total += part;
+    }
+    if (weighted_rank) cands[c].count = n;
+    else cands[c].wcount = total;
 }
 
 // stage-2 reorder by (power desc, index asc): pack to RawCand keys, sort, permute
