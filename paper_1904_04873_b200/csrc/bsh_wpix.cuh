@@ -38,6 +38,8 @@ constexpr int kWpixHeader = 128 + kWpixWarps * kStageSfts * 8;   // mbarriers + 
 // BSH_WPIX_ROLL 1: one copy of the 16-SFT stage code serves both halves of a block of 32 (same speed as two copies, half the
 // code).  Rolling further (groups of 2 / 4 / 8 SFTs) measured 23.4 / 18.8 / 19.1 ms against 15.9 ms on config 2: the
 // look-ahead across the whole stage hides the load and FP64 latencies.
+// Also measured and rejected: 3 bins per byte in alternating bit triples (R2P masks 0x0e / 0x70 write disjoint predicates, so
+// the next R2P can issue before the adds of the previous byte): 30 R2P per triple instead of 15, 17.1 ms.
 #ifndef BSH_WPIX_ROLL
 #define BSH_WPIX_ROLL 1
 #endif
