@@ -57,8 +57,9 @@ SMEM_BYTES_PER_TRIPLE = 12.0 + 4.0 + 4.0      # 96-bit window + D (8 B per 2 tem
 ALU_OPS_PER_TRIPLE = 6.0 + 1.125 + 3.0         # the integer-ALU pipe's share of the above
 GATHER_LANES_PER_SM_CLK = 32                   # north_star bound (b) read literally: one 4-byte lane-gather per accumulation
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
-NCU_DRAM_BYTES = {"weighted": None, "unweighted": None}
-NCU_DRAM_SOURCE = "profiles/ (no capture of this kernel yet)"
+NCU_DRAM_BYTES = {(3, "weighted"): 117.2e6, (2, "weighted"): 9.26e6, (2, "unweighted"): 13.14e6}
+NCU_DRAM_SOURCE = ("profiles/r02_stage1_wpix_full.md, r02_stage1_pix_full.md (config-2 launches, ncu --set full) and "
+                   "profiles/r02_dram_config3.md (config-3 weighted launch, dram metrics only)")
 
 
 def measured_peaks_file():
@@ -384,7 +385,7 @@ def roofline(mode: str, wl, k_ms: float, st: dict, pk: dict) -> dict:
     acc = wl.n_accumulations
     secs = k_ms * 1e-3
     common = {"kernel": kernel_name(st["kernel_variant"], mode == "weighted"), "kernel_ms": k_ms,
-              "traffic": NCU_DRAM_BYTES[mode], "traffic_source": NCU_DRAM_SOURCE,
+              "traffic": NCU_DRAM_BYTES.get((2 if wl.n_sft < 4000 else 3, mode)), "traffic_source": NCU_DRAM_SOURCE,
               "gather_bound": {"note": "north_star bound (b) read literally: one 4-byte shared-memory lane-gather per "
                                        "accumulation at 32 lanes/clk/SM; the 90 f0 bins of a band share each gathered window",
                                "frac": acc / secs / (GATHER_LANES_PER_SM_CLK * per_s)},
