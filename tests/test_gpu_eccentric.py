@@ -109,3 +109,24 @@ def test_eccentric_grid_rejects_bad_pairs(bsh, torch, ctx):
     d_peak = ctx.build_peakgram(d_rho, 1.6)
     with pytest.raises(bsh.BshError):
         ctx.stage1_hough(d_peak, bad, mode=bsh.BSH_UNWEIGHTED, topk=10)
+
+
+def test_eccentric_large_toplist_paths(bsh, torch, ctx):
+    """A toplist of 100 000 entries on an eccentric grid: the radix sort and the one-thread-per-candidate rescoring / stage-2
+    kernels (the large-list path of SURVEY NEXT-1) with the Eq. (14) terms compiled in."""
+    wl = synth.eccentric(synth.noise_workload(seed=21, n_sft=200, n_f0=90, margin=60, f_band_start=150.0, n_pix_side=8,
+                                              ap=(10.0, 40.0), P_days=(15.0, 31.0), n_t=3, topk=100_000),
+                         e_max=0.08, n_e=1, n_omega=3)
+    assert wl.n_templates == 64 * 2 * 2 * 3 * 4 * 90
+    pk = oracle.peakgram(wl.rho)
+    want_n, want_w = oracle.stage1(wl, pk, wl.w, mode=oracle.CANONICAL)
+    n, top = run(bsh, torch, ctx, wl, bsh.BSH_UNWEIGHTED, topk=100_000)
+    assert np.array_equal(n, want_n)
+    order = np.lexsort((np.arange(want_n.size), -want_n.astype(np.int64)))[:100_000]
+    assert np.array_equal(top["index"], order.astype(np.uint64))
+    assert np.array_equal(top["count"], want_n[order])
+    assert np.allclose(top["wcount"], want_w[order], rtol=RTOL, atol=0)
+    assert np.allclose(top["power"], oracle.stage2(wl, top["index"], wl.rho, wl.w), rtol=RTOL, atol=0)
+    w, topw = run(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED, topk=100_000)
+    assert np.array_equal(topw["count"], want_n[topw["index"].astype(np.int64)])
+    assert np.all(np.diff(topw["wcount"]) <= 0)
