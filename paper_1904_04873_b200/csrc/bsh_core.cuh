@@ -451,6 +451,9 @@ BSH_HD int32_t count_at(const Counter<NW, HP> &c, int w, int b)
 // Lean resolution of deferred breaks (used by the pixel-lane kernel, bsh_pix.cuh; __host__ __device__ so that the host
 // emulation test runs the same code).
 // ---------------------------------------------------------------------------------------------------------------------
+#ifndef BSH_FIX_SHORTCUT
+#define BSH_FIX_SHORTCUT 1
+#endif
 BSH_HD float fast_divide(float a, float b)
 {
 #ifdef __CUDA_ARCH__
@@ -476,10 +479,16 @@ BSH_HD Win<NW> exact_window_pos(const TrackConst &tc, const uint4 *row_positions
     const int32_t d = sL - s0;
     if (CLAMP || (d != 1 && d != -1)) return track_window_pos<NW, CLAMP>(tc, row_positions, D, B);
     const float dist = (float)(((double)r0 + (d > 0 ? 0.5 : -0.5)) - y0);     // signed distance to the crossed half-integer
-    int j = (int)ceilf(fast_divide(dist, (float)g));
-    j = j < 1 ? 1 : (j > tc.n_fj - 1 ? tc.n_fj - 1 : j);
-    while (j > 1 && shift_of(dadd(tc.u0, (double)(j - 1)), g, tc.off) != s0) --j;
-    while (j < tc.n_fj - 1 && shift_of(dadd(tc.u0, (double)j), g, tc.off) == s0) ++j;
+    const float t = fast_divide(dist, (float)g);         // the crossing in units of j: y_j = y_0 + j g up to 1e-14
+    int j = (int)ceilf(t);
+    // t carries an FP32 error below 2e-5 (|t| < 2^7, three roundings of 6e-8); when it lies further than 1e-3 from an
+    // integer, ceil(t) IS the first bin with the new shift and the canonical re-evaluation is skipped (99.8 % of breaks)
+    const bool sure = BSH_FIX_SHORTCUT && fabsf(t - rintf(t)) > 1e-3f && j >= 1 && j <= tc.n_fj - 1;
+    if (!sure) {
+        j = j < 1 ? 1 : (j > tc.n_fj - 1 ? tc.n_fj - 1 : j);
+        while (j > 1 && shift_of(dadd(tc.u0, (double)(j - 1)), g, tc.off) != s0) --j;
+        while (j < tc.n_fj - 1 && shift_of(dadd(tc.u0, (double)j), g, tc.off) == s0) ++j;
+    }
     const Win<NW> a = load_position<NW>(row_positions, s0);
     const Win<NW> b = load_position<NW>(row_positions, sL);
     Win<NW> out;
