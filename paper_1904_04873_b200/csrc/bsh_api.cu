@@ -827,13 +827,13 @@ int bsh_normalise_peakgram(bsh_ctx *ctx, const float *d_sft, int32_t n_sft, int3
     if (d_rho && rho_row_stride < K) return fail(ctx, BSH_EINVAL, "rho_row_stride < n_raw - window + 1");
     if (d_peak && (int64_t)words_per_row * 32 < K) return fail(ctx, BSH_ESMALL, "words_per_row * 32 < n_raw - window + 1");
     const DeviceGuard device_guard(ctx->device);
-    int n2 = 32;
-    while (n2 < n_raw) n2 <<= 1;
-    const size_t smem = (size_t)n2 * 8 + (size_t)n_raw * 8;
+    const size_t smem = front_smem_bytes(n_raw);
+    if (smem > 48 * 1024)
+        CK(cudaFuncSetAttribute(normalise_peakgram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     CK(cudaEventRecord(ctx->ev[10], ctx->stream));
     normalise_peakgram_kernel<<<(unsigned)n_sft, kFrontThreads, smem, ctx->stream>>>(
         (const float2 *)d_sft, n_raw, sft_row_stride, window, median_bias, rho_th, d_rho, rho_row_stride, d_peak,
-        words_per_row, n2);
+        words_per_row);
     count_launch(ctx);
     CK(cudaGetLastError());
     CK(cudaEventRecord(ctx->ev[11], ctx->stream));
