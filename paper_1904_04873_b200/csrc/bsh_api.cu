@@ -894,7 +894,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
                                                  ctx->opt_force_clamp != 0, ecc_max);
         const PosGeometry pgw = pos_geometry(tgw, sfts->n_bins, grid->n_f0, nw, tile);
         const WpixStage ws(pgw.n_pos, wpix_entry_bytes(nbytes));
-        const int stages = std::min(kMaxStages, (220 * 1024 - kWpixHeader) / ws.stride);     // one block per SM
+        const int stages = std::min(kMaxStages, ((226 * 1024) / kWpixBlocksPerSm - 2048 - kWpixHeader) / ws.stride);
         if (stages >= 2) {
             pd.use_wpix = true;
             pd.tile_bins = tile; pd.wpix_nbytes = nbytes; pd.NW = nw;

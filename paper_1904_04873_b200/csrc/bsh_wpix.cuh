@@ -32,6 +32,12 @@ namespace bsh {
 #ifndef BSH_WPIX_WARPS
 #define BSH_WPIX_WARPS 12
 #endif
+#ifndef BSH_WPIX_BPS
+#define BSH_WPIX_BPS 1
+#endif
+constexpr int kWpixBlocksPerSm = BSH_WPIX_BPS;       // resident blocks per SM the kernel is built for (measured on config 2: 1 x 12
+                                                     // warps 15.90 ms, 2 x 6 warps 16.16 ms, 3 x 4 warps 15.66 ms -- but with 3 blocks
+                                                     // the wide tables of configs 3 and 5 leave no room for two stages)
 constexpr int kWpixWarps = BSH_WPIX_WARPS;           // warps (= binary templates) per block; one block per SM
 constexpr int kWpixHeader = 128 + kWpixWarps * kStageSfts * 8;   // mbarriers + one B buffer per warp
 
@@ -299,7 +305,7 @@ __device__ __noinline__ Win7<NBYTES> exact_window7(const TrackConst &tc, const u
 }
 
 template <int NBYTES, bool CLAMP>
-__global__ void __launch_bounds__(32 * kWpixWarps, 1) stage1_weighted_pix_kernel(const WpixParams p)
+__global__ void __launch_bounds__(32 * kWpixWarps, kWpixBlocksPerSm) stage1_weighted_pix_kernel(const WpixParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int NB = kWpixBits * NBYTES;
