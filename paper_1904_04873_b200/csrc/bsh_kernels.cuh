@@ -900,8 +900,16 @@ __global__ void __launch_bounds__(256) transpose_cs_kernel(const double2 *__rest
     cs_t[t] = cs[(int64_t)p * n_pad + i];
 }
 
+#ifndef BSH_ROWS_MINB
+#define BSH_ROWS_MINB 8        // 32 registers, 64 warps per SM: the kernels are latency-bound (measured on the N_C = 5 % list of config 2:
+#endif                         // rescoring + stage 2 68 ms at 8 blocks per SM against 80 ms at the 5 the compiler picked; unroll 4 / 6 / 16: 84 / 89 / 89 ms)
+#ifndef BSH_ROWS_UNROLL
+#define BSH_ROWS_UNROLL 8
+#endif
+#define BSH_PRAGMA_(x) _Pragma(#x)
+#define BSH_PRAGMA(x) BSH_PRAGMA_(x)
 template <bool ECC>
-__global__ void __launch_bounds__(256) stage2_rows_kernel(const TrackTables t, const float *__restrict__ rho, int64_t stride,
+__global__ void __launch_bounds__(256, BSH_ROWS_MINB) stage2_rows_kernel(const TrackTables t, const float *__restrict__ rho, int64_t stride,
                                                           const float *__restrict__ w, bsh_cand *__restrict__ cands, int n_cands)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -912,7 +920,7 @@ __global__ void __launch_bounds__(256) stage2_rows_kernel(const TrackTables t, c
     for (int i0 = 0; i0 < t.n_sft; i0 += kRowChunk) {
         const int i1 = i0 + kRowChunk < t.n_sft ? i0 + kRowChunk : t.n_sft;
         float part = 0.0f;
-#pragma unroll 8
+BSH_PRAGMA(unroll BSH_ROWS_UNROLL)
         for (int i = i0; i < i1; ++i) {                   // (unrolled: the loads of 8 SFTs are in flight together)
             const int col = track_column<ECC>(k, i, t.n_bins);
             const float r = __ldg(rho + (int64_t)i * stride + (col >= 0 ? col : 0));
@@ -925,7 +933,7 @@ __global__ void __launch_bounds__(256) stage2_rows_kernel(const TrackTables t, c
 }
 
 template <bool ECC>
-__global__ void __launch_bounds__(256) rescore_rows_kernel(const TrackTables t, const uint32_t *__restrict__ peak,
+__global__ void __launch_bounds__(256, BSH_ROWS_MINB) rescore_rows_kernel(const TrackTables t, const uint32_t *__restrict__ peak,
                                                            int words_per_row, const float *__restrict__ w, int weighted_rank,
                                                            bsh_cand *__restrict__ cands, int n_cands)
 {
@@ -938,7 +946,7 @@ __global__ void __launch_bounds__(256) rescore_rows_kernel(const TrackTables t, 
     for (int i0 = 0; i0 < t.n_sft; i0 += kRowChunk) {
         const int i1 = i0 + kRowChunk < t.n_sft ? i0 + kRowChunk : t.n_sft;
         float part = 0.0f;
-#pragma unroll 8
+BSH_PRAGMA(unroll BSH_ROWS_UNROLL)
         for (int i = i0; i < i1; ++i) {
             const int col = track_column<ECC>(k, i, t.n_bins);
             const uint32_t word = __ldg(peak + (int64_t)i * words_per_row + ((col >= 0 ? col : 0) >> 5));
