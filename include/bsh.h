@@ -39,6 +39,7 @@ extern "C" {
 #define BSH_ESMALL   -4   /* an output buffer is too small (e.g. words_per_row * 32 < n_bins)                    */
 #define BSH_ESTATE   -5   /* call order violated (e.g. bsh_stage1_collect without bsh_stage1_launch), or the candidate  */
                           /* selection did not converge (degenerate input); message in bsh_last_error              */
+#define BSH_ELIMIT   -6   /* a list is longer than the fixed scratch of bsh_post_coincidences_static holds               */
 
 /* mode bits for stage 1 */
 #define BSH_UNWEIGHTED 0  /* rank by the integer number count n                                   (L223)         */
@@ -227,6 +228,49 @@ typedef struct {
  * *h_n_pairs receives the number found (may exceed max_pairs: call again with larger buffers). */
 int bsh_post_coincidences(bsh_ctx *ctx, const bsh_candset *a, const bsh_candset *b, double window, int64_t max_pairs,
                           int32_t *d_pair_a, int32_t *d_pair_b, double *d_centroid, double *d_pair_sig, int64_t *h_n_pairs);
+
+/* bsh_post_coincidences without any allocation -- for callers that must not, or cannot, allocate device memory.
+ *
+ * Who that is.  bsh_post_coincidences keeps its work area (the bit matrix "pair (a, b) is closer than the window", the
+ * per-row pair counts and their prefix sums) in cudaMalloc'ed buffers that its context grows on demand.  That is wrong
+ * for three kinds of user of this library:
+ *   - a search job that has handed the whole of the GPU's memory to a pool of its own (a framework's caching allocator, a
+ *     batch scheduler's fixed per-job share of a GPU that several jobs use): the library's own cudaMalloc then fails, or
+ *     takes memory the job was promised;
+ *   - the follow-up stage of a sweep that still has stage-1 kernels of other sky patches running on other streams:
+ *     cudaMalloc and cudaFree make the whole device wait, so a growing work area stalls every one of those patches;
+ *   - a monitoring / low-latency consumer of the toplists that has to answer in bounded time: an allocation takes an
+ *     unbounded time and can fail at a moment when nothing can be done about it.
+ * This call therefore takes no bsh_ctx (creating one allocates events and pinned memory) and calls no cudaMalloc, cudaFree,
+ * cudaMallocHost or any other allocating routine: inputs and outputs are the caller's, and the work area is ONE array that is
+ * part of the loaded library image on every GPU, BSH_STATIC_SCRATCH_BYTES (about 8.1 MiB) per GPU from the moment the
+ * library is loaded there until the process exits, whether or not this call is ever made.
+ *
+ * Limit.  a->n <= BSH_STATIC_MAX_CANDS and b->n <= BSH_STATIC_MAX_CANDS (8192; the paper's final toplists hold 5000
+ * candidates, L496).  Longer lists are refused with BSH_ELIMIT before anything is launched -- use
+ * bsh_post_coincidences for those.
+ *
+ * Arguments and results are those of bsh_post_coincidences (same kernels, same operation order: the pair list, centroids
+ * and significances are bit-identical), except:
+ *   device, cuda_stream   the GPU and the cudaStream_t (NULL = legacy default stream) to run on, in place of the context
+ *   h_err, err_len        optional caller's buffer that receives a NUL-terminated description when the result is not
+ *                         BSH_OK (h_err may be NULL)
+ * Synchronous: the stream is synchronised before the call returns.
+ *
+ * First call on each device: it looks up the device address of the work area (cudaGetSymbolAddress; this also makes the
+ * CUDA runtime load the library's device code onto that GPU if nothing did so before) and remembers it.  Make that first
+ * call during set-up, before any stream capture is begun; later calls on that device do no look-up.
+ *
+ * Sharing.  Every call on a device -- from any stream and any host thread of the process -- uses the same work area, and
+ * the area keeps what the previous call left in it (the call clears the part that has to start at zero, the row counts;
+ * everything else it reads it has first overwritten itself).  Two calls whose kernels can be on the same GPU at the same
+ * time therefore corrupt each other's results: the caller runs them one after the other.  (Calls on different GPUs, and
+ * calls in different processes, do not share anything.) */
+#define BSH_STATIC_MAX_CANDS     8192
+#define BSH_STATIC_SCRATCH_BYTES (65792 + 32768 + 8192 * (8192 / 32) * 4)
+int bsh_post_coincidences_static(int device, void *cuda_stream, const bsh_candset *a, const bsh_candset *b, double window,
+                                 int64_t max_pairs, int32_t *d_pair_a, int32_t *d_pair_b, double *d_centroid,
+                                 double *d_pair_sig, int64_t *h_n_pairs, char *h_err, int32_t err_len);
 
 /* Steps 2-3 (L401-L405): clusters = connected components of the graph d < window; d_label[i] = smallest index of the
  * members of i's cluster.  prune_window > 0 (option B, L403): members at that distance or further from the cluster's top

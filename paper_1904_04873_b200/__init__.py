@@ -8,7 +8,8 @@ but creating a Context without a CUDA device raises.
 from . import binding
 from .binding import (BSH_FAMILY_AUTO, BSH_FAMILY_PIXEL_LANE, BSH_FAMILY_TEMPLATE_LANE, BSH_FAMILY_WINDOW, BSH_NAIVE,
                       BSH_OPT_FORCE_CLAMP, BSH_OPT_KERNEL_FAMILY, BSH_OPT_PIXELS_PER_THREAD, BSH_UNWEIGHTED, BSH_WEIGHTED,
-                      CAND_DTYPE, BshError, Context, Stats, library, template_decode, template_index)
+                      CAND_DTYPE, BshError, Context, Stats, library, post_coincidences_static, template_decode,
+                      template_index)
 
 __all__ = ["Context", "BshError", "Stats", "library", "CAND_DTYPE", "BSH_UNWEIGHTED", "BSH_WEIGHTED", "BSH_NAIVE",
-           "template_index", "template_decode"]
+           "template_index", "template_decode", "post_coincidences_static"]

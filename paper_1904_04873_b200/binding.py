@@ -16,7 +16,8 @@ BSH_FAMILY_AUTO, BSH_FAMILY_PIXEL_LANE, BSH_FAMILY_TEMPLATE_LANE, BSH_FAMILY_WIN
 EXPORTS = ["bsh_version", "bsh_create", "bsh_destroy", "bsh_last_error", "bsh_get_stats", "bsh_set_option",
            "bsh_measure_peaks", "bsh_build_peakgram", "bsh_normalise_peakgram", "bsh_median_bias",
            "bsh_stage1_hough", "bsh_stage1_launch", "bsh_stage1_collect", "bsh_stage2_power", "bsh_search_patch_host",
-           "bsh_template_index", "bsh_template_decode", "bsh_template_index_ecc", "bsh_template_decode_ecc", "bsh_post_coincidences", "bsh_post_cluster"]
+           "bsh_template_index", "bsh_template_decode", "bsh_template_index_ecc", "bsh_template_decode_ecc", "bsh_post_coincidences", "bsh_post_cluster",
+           "bsh_post_coincidences_static"]
 
 # numpy view of bsh_cand (24 bytes)
 CAND_DTYPE = np.dtype([("index", "<u8"), ("count", "<i4"), ("wcount", "<f4"), ("power", "<f4"), ("flags", "<u4")])
@@ -130,6 +131,48 @@ def template_decode(wl, index):
     out = [C.c_int32() for _ in range(5)]
     library().bsh_template_decode(C.byref(_Problem(wl).grid), C.c_uint64(int(index)), *[C.byref(o) for o in out])
     return tuple(o.value for o in out)
+
+
+STATIC_MAX_CANDS = 8192        # BSH_STATIC_MAX_CANDS of include/bsh.h
+
+
+def post_coincidences_static(a, b, window: float, out, device: int = 0, stream=None):
+    """bsh_post_coincidences_static: the coincidence step (Eq. 44) for callers that cannot allocate device memory
+    -- the GPU's memory belongs to somebody else's pool, other patches' kernels are running and must not be stalled by a
+    cudaMalloc, or the answer is needed in bounded time (include/bsh.h gives the full account).  No Context is involved and
+    the library allocates nothing: its work area is a fixed array inside the loaded library, which limits each list to
+    STATIC_MAX_CANDS = 8192 candidates (BshError with code -6 beyond that) and means that two such calls must never run on
+    one GPU at the same time.  This wrapper allocates nothing either.
+
+    a, b: (d_param [n, 6], d_res [n, 6], d_sig [n]) CUDA float64 tensors on `device`.
+    out:  the caller's result buffers (pair_a int32 [cap], pair_b int32 [cap], centroid float64 [cap, 6], significance
+          float64 [cap]) on `device`; at most cap pairs are written.
+    stream: a torch.cuda.Stream, or None for the legacy default stream.
+    Returns the number of pairs found (it may exceed cap).  The first call on a device also looks up the work area's address;
+    make it at set-up time, before any stream capture."""
+    import torch
+    lib = library()
+    pa, pb, cen, sig = out
+    cap = int(pa.shape[0])
+    assert pa.is_cuda and pa.dtype == torch.int32 and pb.dtype == torch.int32 and int(pb.shape[0]) == cap
+    assert cen.dtype == torch.float64 and tuple(cen.shape) == (cap, 6) and sig.dtype == torch.float64 and int(sig.shape[0]) == cap
+    assert all(t.is_contiguous() and t.is_cuda for t in out)
+    sets = []
+    for d_param, d_res, d_sig in (a, b):
+        n = int(d_param.shape[0])
+        for t, shape in ((d_param, (n, 6)), (d_res, (n, 6)), (d_sig, (n,))):
+            assert t.is_cuda and t.dtype == torch.float64 and tuple(t.shape) == shape and t.is_contiguous()
+        sets.append(_CandSet(n=n, d_param=d_param.data_ptr() if n else None, d_res=d_res.data_ptr() if n else None,
+                             d_sig=d_sig.data_ptr() if n else None))
+    n_pairs = C.c_int64(0)
+    err = C.create_string_buffer(512)
+    rc = lib.bsh_post_coincidences_static(C.c_int(device), C.c_void_p(stream.cuda_stream if stream is not None else None),
+                                          C.byref(sets[0]), C.byref(sets[1]), C.c_double(window), C.c_int64(cap),
+                                          C.c_void_p(pa.data_ptr()), C.c_void_p(pb.data_ptr()), C.c_void_p(cen.data_ptr()),
+                                          C.c_void_p(sig.data_ptr()), C.byref(n_pairs), err, C.c_int32(len(err)))
+    if rc != 0:
+        raise BshError(f"bsh error {rc}: {err.value.decode()}")
+    return int(n_pairs.value)
 
 
 class Context:

@@ -9,6 +9,7 @@
 
 #include <algorithm>
 #include <chrono>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1358,3 +1359,109 @@ void bsh_template_decode(const bsh_grid *g, uint64_t idx, int32_t *pix, int32_t 
 }
 
 }  // extern "C"
+
+// =====================================================================================================================
+// bsh_post_coincidences_static: step 1 of the post-processing with its work area in the library image (include/bsh.h says
+// for whom and why).  Nothing below allocates: no cudaMalloc / cudaFree / cudaMallocHost, no std::string or std::vector.
+// =====================================================================================================================
+namespace {
+
+constexpr int kStaticMaxCands = BSH_STATIC_MAX_CANDS;
+constexpr int kStaticMaxDevices = 64;
+// layout of the work area (every part on a 256-byte boundary):  prefix sums [n_a + 1] int64 | row counts [n_a] int32 |
+// bit matrix [n_a][ceil(n_b / 32)] uint32
+constexpr size_t kStaticOffBytes = ((size_t)(kStaticMaxCands + 1) * 8 + 255) / 256 * 256;
+constexpr size_t kStaticCntBytes = (size_t)kStaticMaxCands * 4;
+constexpr size_t kStaticAdjBytes = (size_t)kStaticMaxCands * (kStaticMaxCands / 32) * 4;
+static_assert(kStaticOffBytes + kStaticCntBytes + kStaticAdjBytes == (size_t)BSH_STATIC_SCRATCH_BYTES, "bsh.h states the size");
+static_assert(kStaticCntBytes % 256 == 0 && kStaticMaxCands % 32 == 0, "alignment of the parts");
+
+// One copy per GPU that loads this library, for the life of the process.  In HOST code the name `g_static_scratch` is only
+// a handle for the runtime's symbol calls, not a device address: the kernels are given the pointer cudaGetSymbolAddress
+// returns for the current device (static_scratch_of below), never the name.
+static __device__ __align__(256) unsigned char g_static_scratch[BSH_STATIC_SCRATCH_BYTES];
+
+std::mutex g_static_mutex;
+unsigned char *g_static_ptr[kStaticMaxDevices] = {};      // device address of g_static_scratch on each GPU, once looked up
+
+int static_fail(char *h_err, int32_t err_len, int code, const char *fmt, ...)
+{
+    if (h_err && err_len > 0) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(h_err, (size_t)err_len, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+// `device` must be the current device.  The first call per device does the look-up; the answer never changes afterwards.
+int static_scratch_of(int device, unsigned char **out, char *h_err, int32_t err_len)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess || !p)
+            return static_fail(h_err, err_len, BSH_ECUDA, "bsh_post_coincidences_static: cudaGetSymbolAddress on device %d failed: %s",
+                               device, cudaGetErrorString(e));
+        g_static_ptr[device] = (unsigned char *)p;
+    }
+    *out = g_static_ptr[device];
+    return BSH_OK;
+}
+
+#define CKS(call)                                                                                                  \
+    do {                                                                                                           \
+        cudaError_t e_ = (call);                                                                                   \
+        if (e_ != cudaSuccess)                                                                                     \
+            return static_fail(h_err, err_len, BSH_ECUDA, "bsh_post_coincidences_static: %s failed: %s", #call,   \
+                               cudaGetErrorString(e_));                                                            \
+    } while (0)
+
+bool static_candset_ok(const bsh_candset *c) { return c && c->n >= 0 && (c->n == 0 || (c->d_param && c->d_res && c->d_sig)); }
+
+}  // namespace
+
+extern "C" int bsh_post_coincidences_static(int device, void *cuda_stream, const bsh_candset *a, const bsh_candset *b,
+                                            double window, int64_t max_pairs, int32_t *d_pair_a, int32_t *d_pair_b,
+                                            double *d_centroid, double *d_pair_sig, int64_t *h_n_pairs, char *h_err,
+                                            int32_t err_len)
+{
+    if (h_err && err_len > 0) h_err[0] = 0;
+    if (!static_candset_ok(a) || !static_candset_ok(b))
+        return static_fail(h_err, err_len, BSH_EINVAL, "bsh_post_coincidences_static: bad candidate set");
+    if (!h_n_pairs || max_pairs < 0 || !(window > 0.0) || (max_pairs > 0 && (!d_pair_a || !d_pair_b || !d_centroid || !d_pair_sig)))
+        return static_fail(h_err, err_len, BSH_EINVAL, "bsh_post_coincidences_static: bad arguments");
+    *h_n_pairs = 0;
+    if (a->n > kStaticMaxCands || b->n > kStaticMaxCands)
+        return static_fail(h_err, err_len, BSH_ELIMIT,
+                           "bsh_post_coincidences_static: lists of %d and %d candidates, the fixed work area holds at most %d "
+                           "per list (BSH_STATIC_MAX_CANDS); use bsh_post_coincidences for longer lists",
+                           a->n, b->n, kStaticMaxCands);
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1 || device < 0 || device >= n_dev || device >= kStaticMaxDevices)
+        return static_fail(h_err, err_len, BSH_ECUDA, "bsh_post_coincidences_static: no CUDA device %d", device);
+    if (a->n == 0 || b->n == 0) return BSH_OK;
+    const DeviceGuard device_guard(device);
+    unsigned char *scratch = nullptr;
+    TRY(static_scratch_of(device, &scratch, h_err, err_len));
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    int64_t *d_off = (int64_t *)scratch;
+    int32_t *d_cnt = (int32_t *)(scratch + kStaticOffBytes);
+    uint32_t *d_adj = (uint32_t *)(scratch + kStaticOffBytes + kStaticCntBytes);
+    const int words = (b->n + 31) / 32;
+    // the work area still holds the previous call's contents: the row counts are accumulated with atomicAdd and must start
+    // at zero; d_adj [n_a][words] and d_off [n_a + 1] are written in full by the kernels below before they are read
+    CKS(cudaMemsetAsync(d_cnt, 0, (size_t)a->n * 4, stream));
+    const int64_t warps = (int64_t)a->n * words;
+    post_adjacency_kernel<<<(unsigned)((warps + 7) / 8), 256, 0, stream>>>(a->n, a->d_param, a->d_res, b->n, b->d_param, b->d_res,
+                                                                          window * window, 0, words, d_adj, d_cnt);
+    post_scan_kernel<<<1, 1024, 0, stream>>>(a->n, d_cnt, d_off);
+    post_pairs_kernel<<<(a->n + 255) / 256, 256, 0, stream>>>(a->n, words, d_adj, d_off, a->d_param, a->d_sig, b->d_param, b->d_sig,
+                                                             max_pairs, d_pair_a, d_pair_b, d_centroid, d_pair_sig);
+    CKS(cudaGetLastError());
+    CKS(cudaMemcpyAsync(h_n_pairs, d_off + a->n, 8, cudaMemcpyDeviceToHost, stream));
+    CKS(cudaStreamSynchronize(stream));
+    return BSH_OK;
+}
