@@ -57,6 +57,13 @@ extern "C" {
 #define BSH_FAMILY_TEMPLATE_LANE 2     /* binary templates on the lanes, position table (bsh_pos.cuh)              */
 #define BSH_FAMILY_WINDOW      3       /* binary templates on the lanes, funnel-shift window table (wide slabs)    */
 
+/* bsh_stats.kernel_variant / 1000: the accumulation kernel that ran.  A separate numbering from BSH_FAMILY_* on purpose:
+ * a family is what the caller may ask for, a kernel id says what was launched (the pixel-lane family has two kernels). */
+#define BSH_KERNEL_WINDOW         0    /* funnel-shift window table           (BSH_FAMILY_WINDOW)                          */
+#define BSH_KERNEL_TEMPLATE_LANE  1    /* position table, templates on lanes  (BSH_FAMILY_TEMPLATE_LANE)                   */
+#define BSH_KERNEL_PIXEL_LANE     2    /* unweighted pixel-lane kernel        (BSH_FAMILY_PIXEL_LANE, BSH_UNWEIGHTED)      */
+#define BSH_KERNEL_PIXEL_LANE_W   3    /* weighted pixel-lane kernel          (BSH_FAMILY_PIXEL_LANE, BSH_WEIGHTED)        */
+
 typedef struct bsh_ctx bsh_ctx;
 
 /* One SFT set.  Stage 1 and stage 2 may be given different sets (the paper's stage 2 adds half-overlapped SFTs,
@@ -77,8 +84,8 @@ typedef struct {
 /* One sky patch x template grid. */
 typedef struct {
     int32_t n_pix;  const double *h_alpha, *h_delta;  /* [n_pix] right ascension / declination, radians           */
-    int64_t k_band0;                                  /* f0_j = (k_band0 + j) / T, j = 0 .. n_f0-1 (R-3);          */
-    int32_t n_f0;                                     /*   requires k_band0 >= k_slab0                             */
+    int64_t k_band0;                                  /* f0_j = (k_band0 + j) / T, j = 0 .. n_f0-1 (R-3); requires */
+    int32_t n_f0;                                     /*   k_slab0 <= k_band0 <= k_slab0 + 2^24, k_band0 + n_f0 < 2^32 */
     int32_t n_ap;   const double *h_ap;               /* [n_ap]  projected semi-major axis, light-seconds (L70)    */
     int32_t n_P;    const double *h_P;                /* [n_P]   orbital period, seconds                           */
     int32_t n_tasc; const double *h_tasc_frac;        /* [n_tasc] t_asc = t_search_mid + frac * P (Eq. 35, R-13)   */
@@ -109,8 +116,8 @@ typedef struct {
     int64_t  n_candidates;       /* templates that passed the in-kernel threshold                                  */
     double   threshold;          /* final in-kernel threshold (count or weighted count)                            */
     int32_t  n_passes;           /* accumulation passes (1 unless the threshold had to be moved)                   */
-    int32_t  kernel_variant;     /* family * 1000 + words * 100 + pixels_per_thread * 10 + clamp; family 3 = weighted  */
-                                 /* pixel-lane, 2 = pixel-lane, 1 = template-lane position table, 0 = funnel-shift     */
+    int32_t  kernel_variant;     /* kernel * 1000 + words * 100 + pixels_per_thread * 10 + clamp; kernel = one of the  */
+                                 /* BSH_KERNEL_* ids below (which accumulation kernel RAN; not a BSH_FAMILY_* request) */
     int32_t  threads_per_block;  /* of the accumulation kernel                                                     */
     int32_t  grid_blocks;        /* of the accumulation kernel                                                     */
     int64_t  launches;           /* kernels launched by this context since creation                                */
@@ -182,7 +189,9 @@ double bsh_median_bias(int32_t window);    /* sum_{i = (window + 1) / 2}^{window
  * A track leaving the slab is not an error: that SFT contributes 0 (R-6).
  * bsh_stage1_hough = bsh_stage1_launch + bsh_stage1_collect; it returns with d_top complete (stream synchronised).
  * bsh_stage1_launch is asynchronous (no host synchronisation); bsh_stage1_collect synchronises the stream, runs the
- * selection, and leaves the toplist writes enqueued on the stream (h_n_top is final on return).  Between launch and
+ * selection, and leaves the toplist writes enqueued on the stream (h_n_top is final on return).  The wcount of every
+ * toplist entry is re-scored in a fixed order that does not depend on the accumulation kernel, the two orders given at
+ * bsh_stage2_power (block per entry up to 65536 entries, thread per entry beyond).  Between launch and
  * collect the caller may enqueue work on OTHER contexts/streams (this is how config 5 overlaps two patches).
  * The host arrays inside `sfts` and `grid` are read during launch only; the DEVICE buffers d_peak, sfts->d_w and
  * d_counts_full are read / written until bsh_stage1_collect returns (toplist rescoring and threshold retries) and must stay
@@ -196,9 +205,14 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
 int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top);
 
 /* Stage 2 (Eq. 26): power[c] = sum_i w_i rho[i][k_i] along the track of d_cands[c].index over the SFT set
- * `sfts` (FP32 products; thread t of the candidate's 128-thread block sums SFTs t, t + 128, ... in order, then a fixed shuffle
- * tree per warp and the warp partials in warp order; R-20), written into
- * d_cands[c].power.  If sort_by_power != 0 the records are then reordered by (power desc, index asc).
+ * `sfts`, written into d_cands[c].power.  If sort_by_power != 0 the records are then reordered by (power desc, index asc).
+ * FP32 summation order (R-20; deterministic run to run, but it DEPENDS ON THE LIST LENGTH):
+ *   n_cands <= 65536   one 128-thread block per candidate: thread t sums the products of SFTs t, t + 128, ... in order, then
+ *                      a fixed xor-shuffle tree per warp, then the four warp partials in warp order;
+ *   n_cands  > 65536   one thread per candidate: partial sums over chunks of 128 consecutive SFTs in SFT order, then the
+ *                      partials in chunk order.
+ * The power of one template can therefore differ in its last bits between a short and a long list (both are within the
+ * 1e-5 relative tolerance of the FP64 sum); the same holds for the wcount that bsh_stage1_collect re-scores.
  * d_rho: [n_sft][rho_row_stride] FP32.  Asynchronous. */
 int bsh_stage2_power(bsh_ctx *ctx, const float *d_rho, int64_t rho_row_stride, const bsh_sfts *sfts,
                      const bsh_grid *grid, bsh_cand *d_cands, int32_t n_cands, int32_t sort_by_power);

@@ -208,6 +208,13 @@ class Context:
         if rc != 0:
             raise BshError(f"bsh error {rc}: {self.lib.bsh_last_error(self._ctx).decode()}")
 
+    def _empty(self, shape, dtype):
+        """An output buffer for the library: on the context's device (not torch's current one) and allocated under the
+        context's stream, the stream the kernels write it on, so that the caching allocator's reuse rules follow that stream."""
+        torch = self.torch
+        with torch.cuda.stream(self.stream):
+            return torch.empty(shape, dtype=dtype, device=f"cuda:{self.device}")
+
     # ---- the three calls of the path -------------------------------------------------------------------------------
     def build_peakgram(self, d_rho, rho_th: float = 1.6, out=None):
         """d_rho: CUDA float32 [N, K] (row stride = d_rho.stride(0)).  Returns CUDA int32 tensor [N, ceil(K/32)] holding
@@ -217,7 +224,7 @@ class Context:
         n, k = d_rho.shape
         wpr = (k + 31) // 32
         if out is None:
-            out = torch.empty((n, wpr), dtype=torch.int32, device=d_rho.device)
+            out = self._empty((n, wpr), torch.int32)
         self._check(self.lib.bsh_build_peakgram(self._ctx, C.c_void_p(d_rho.data_ptr()), C.c_int32(n), C.c_int32(k),
                                                 C.c_int64(d_rho.stride(0)), C.c_float(rho_th), C.c_void_p(out.data_ptr()),
                                                 C.c_int32(out.shape[1])))
@@ -231,8 +238,8 @@ class Context:
         n, n_raw = d_sft.shape
         k = n_raw - window + 1
         b = median_bias(window) if bias is None else bias
-        d_rho = torch.empty((n, k), dtype=torch.float32, device=d_sft.device) if want_rho else None
-        d_peak = torch.empty((n, (k + 31) // 32), dtype=torch.int32, device=d_sft.device) if want_peak else None
+        d_rho = self._empty((n, k), torch.float32) if want_rho else None
+        d_peak = self._empty((n, (k + 31) // 32), torch.int32) if want_peak else None
         self._check(self.lib.bsh_normalise_peakgram(
             self._ctx, C.c_void_p(d_sft.data_ptr()), C.c_int32(n), C.c_int32(n_raw), C.c_int64(d_sft.stride(0)),
             C.c_int32(window), C.c_float(b), C.c_float(rho_th), C.c_void_p(d_rho.data_ptr() if want_rho else None),
@@ -251,8 +258,7 @@ class Context:
     def stage1_collect(self):
         torch = self.torch
         pb, topk = self._pending
-        with torch.cuda.stream(self.stream):             # the records are written on the context's stream
-            d_top = torch.empty(topk * CAND_DTYPE.itemsize, dtype=torch.uint8, device=f"cuda:{self.device}")
+        d_top = self._empty(topk * CAND_DTYPE.itemsize, torch.uint8)
         n_top = C.c_int32(0)
         self._check(self.lib.bsh_stage1_collect(self._ctx, C.c_void_p(d_top.data_ptr()), C.byref(n_top)))
         return d_top, int(n_top.value)
@@ -262,7 +268,7 @@ class Context:
         torch = self.torch
         pb = _Problem(wl, d_w)
         topk = int(topk if topk is not None else wl.topk)
-        d_top = torch.empty(topk * CAND_DTYPE.itemsize, dtype=torch.uint8, device=f"cuda:{self.device}")
+        d_top = self._empty(topk * CAND_DTYPE.itemsize, torch.uint8)
         n_top = C.c_int32(0)
         self._check(self.lib.bsh_stage1_hough(self._ctx, C.c_void_p(d_peak.data_ptr()), C.c_int32(d_peak.shape[1]),
                                               C.byref(pb.sfts), C.byref(pb.grid), C.c_int32(mode), C.c_int32(topk),
@@ -307,10 +313,8 @@ class Context:
         ca, cb = self._candset(*a), self._candset(*b)
         cap = int(max_pairs if max_pairs is not None else max(1, min(ca.n * cb.n, 1 << 22)))
         while True:
-            pa = torch.empty(cap, dtype=torch.int32, device="cuda")
-            pb = torch.empty(cap, dtype=torch.int32, device="cuda")
-            cen = torch.empty((cap, 6), dtype=torch.float64, device="cuda")
-            sig = torch.empty(cap, dtype=torch.float64, device="cuda")
+            pa, pb = self._empty(cap, torch.int32), self._empty(cap, torch.int32)
+            cen, sig = self._empty((cap, 6), torch.float64), self._empty(cap, torch.float64)
             n = C.c_int64(0)
             self._check(self.lib.bsh_post_coincidences(self._ctx, C.byref(ca), C.byref(cb), C.c_double(window), C.c_int64(cap),
                                                        C.c_void_p(pa.data_ptr()), C.c_void_p(pb.data_ptr()),
@@ -325,11 +329,8 @@ class Context:
         torch = self.torch
         c = self._candset(*cands)
         n = max(c.n, 1)
-        label = torch.empty(n, dtype=torch.int32, device="cuda")
-        root = torch.empty(n, dtype=torch.int32, device="cuda")
-        members = torch.empty(n, dtype=torch.int32, device="cuda")
-        cen = torch.empty((n, 6), dtype=torch.float64, device="cuda")
-        sig = torch.empty(n, dtype=torch.float64, device="cuda")
+        label, root, members = (self._empty(n, torch.int32) for _ in range(3))
+        cen, sig = self._empty((n, 6), torch.float64), self._empty(n, torch.float64)
         nc, best = C.c_int32(0), C.c_int32(-1)
         self._check(self.lib.bsh_post_cluster(self._ctx, C.byref(c), C.c_double(window), C.c_double(prune_window),
                                               C.c_void_p(label.data_ptr()), C.c_void_p(root.data_ptr()),

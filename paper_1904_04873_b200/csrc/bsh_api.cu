@@ -30,6 +30,7 @@ namespace {
 
 constexpr unsigned int kCandCap = 1u << 20;      // candidate buffer entries (16 MB)
 constexpr int kMaxPasses = 12;
+constexpr int32_t kMaxTopk = 1 << 27;            // bsh.h: 1 <= topk <= 2^27 (also the largest candidate buffer)
 
 struct DevBuf {
     void *p = nullptr;
@@ -191,8 +192,11 @@ int validate(bsh_ctx *ctx, const bsh_sfts *s, const bsh_grid *g)
         !g->h_ap || !g->h_P || !g->h_tasc_frac)
         return fail(ctx, BSH_EINVAL, "bad grid");
     if (g->k_band0 < s->k_slab0) return fail(ctx, BSH_EINVAL, "k_band0 < k_slab0");
-    if (g->k_band0 - s->k_slab0 > (1 << 24) || g->k_band0 + g->n_f0 >= (1ll << 40))
-        return fail(ctx, BSH_EINVAL, "band offset out of range");
+    // k_band0 + n_f0 < 2^32: the break fix-up of bsh_core.cuh (exact_window_pos) estimates the break bin from
+    // y_0 + j g, which differs from the canonical fl(fl(u_0 + j) g) by up to u 2^-52 bins of j; below 2^32 that is
+    // < 1e-6, far inside its 1e-3 guard (R-7).  2^32 bins is 4.8 MHz at T = 900 s.
+    if (g->k_band0 - s->k_slab0 > (1 << 24) || g->k_band0 + g->n_f0 >= (1ll << 32))
+        return fail(ctx, BSH_EINVAL, "band offset out of range (k_band0 - k_slab0 <= 2^24, k_band0 + n_f0 < 2^32)");
     for (int p = 0; p < g->n_P; ++p)
         if (!(g->h_P[p] > 0)) return fail(ctx, BSH_EINVAL, "P[%d] <= 0", p);
     if (g->n_ecc < 0 || (g->n_ecc > 0 && (!g->h_ecosw || !g->h_esinw))) return fail(ctx, BSH_EINVAL, "bad eccentricity axis");
@@ -848,6 +852,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     if (!ctx) return BSH_EINVAL;
     TRY(validate(ctx, sfts, grid));
     if (!d_peak || topk < 1) return fail(ctx, BSH_EINVAL, "bsh_stage1: null peakgram or topk < 1");
+    if (topk > kMaxTopk) return fail(ctx, BSH_EINVAL, "bsh_stage1: topk = %d is beyond the documented maximum of 2^27", topk);
     if ((int64_t)words_per_row * 32 < sfts->n_bins) return fail(ctx, BSH_ESMALL, "words_per_row * 32 < n_bins");
     if ((mode & BSH_WEIGHTED) && !sfts->d_w) return fail(ctx, BSH_EINVAL, "BSH_WEIGHTED needs sfts->d_w");
     if (mode & ~(BSH_WEIGHTED | BSH_NAIVE)) return fail(ctx, BSH_EINVAL, "unknown mode bits");
@@ -1042,7 +1047,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
 
     ctx->st.n_templates = (int64_t)pd.n_templates;
     ctx->st.n_accumulations = (int64_t)pd.n_templates * sfts->n_sft;
-    ctx->st.kernel_variant = (pd.use_wpix ? 3000 : pd.use_pix ? 2000 : pd.use_pos ? 1000 : 0) + pd.NW * 100 + pd.R * 10 + (pd.clamp ? 1 : 0);
+    ctx->st.kernel_variant = 1000 * (pd.use_wpix ? BSH_KERNEL_PIXEL_LANE_W : pd.use_pix ? BSH_KERNEL_PIXEL_LANE : pd.use_pos ? BSH_KERNEL_TEMPLATE_LANE : BSH_KERNEL_WINDOW) + pd.NW * 100 + pd.R * 10 + (pd.clamp ? 1 : 0);
     return BSH_OK;
 }
 
@@ -1207,6 +1212,7 @@ int bsh_search_patch_host(bsh_ctx *ctx, const float *h_rho, const float *h_w, fl
     if (!ctx) return BSH_EINVAL;
     TRY(validate(ctx, sfts, grid));
     if (!h_rho || !h_top || !h_n_top || topk < 1) return fail(ctx, BSH_EINVAL, "bsh_search_patch_host: bad arguments");
+    if (topk > kMaxTopk) return fail(ctx, BSH_EINVAL, "bsh_search_patch_host: topk = %d is beyond the documented maximum of 2^27", topk);
     if ((mode & BSH_WEIGHTED) && !h_w) return fail(ctx, BSH_EINVAL, "BSH_WEIGHTED needs h_w");
     const DeviceGuard device_guard(ctx->device);
     const int N = sfts->n_sft, K = sfts->n_bins, W = (K + 31) / 32;

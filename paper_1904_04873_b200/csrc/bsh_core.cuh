@@ -481,8 +481,12 @@ BSH_HD Win<NW> exact_window_pos(const TrackConst &tc, const uint4 *row_positions
     const float dist = (float)(((double)r0 + (d > 0 ? 0.5 : -0.5)) - y0);     // signed distance to the crossed half-integer
     const float t = fast_divide(dist, (float)g);         // the crossing in units of j: y_j = y_0 + j g up to 1e-14
     int j = (int)ceilf(t);
-    // t carries an FP32 error below 2e-5 (|t| < 2^7, three roundings of 6e-8); when it lies further than 1e-3 from an
-    // integer, ceil(t) IS the first bin with the new shift and the canonical re-evaluation is skipped (99.8 % of breaks)
+    // Error of t against the true crossing of the canonical y_j = fl(fl(u_0 + j) g), in bins of j (|t| < 2^7):
+    //   FP32: the two conversions and the division, __fdividef being good to 2 ulp: (1 + 1 + 2) 6e-8 2^7 < 4e-5;
+    //   FP64: y_0 and y_j each carry a rounding of <= |y| 2^-53, and so does forming dist; divided by |g| that is
+    //         <= 3 u 2^-53 < 1e-6 for u < 2^32 (validate() in bsh_api.cu enforces k_band0 + n_f0 < 2^32).
+    // Together < 5e-5, a twentieth of the guard: when t lies further than 1e-3 from an integer, ceil(t) IS the first bin
+    // with the new shift and the canonical re-evaluation is skipped (99.8 % of breaks); otherwise it is re-evaluated.
     const bool sure = BSH_FIX_SHORTCUT && fabsf(t - rintf(t)) > 1e-3f && j >= 1 && j <= tc.n_fj - 1;
     if (!sure) {
         j = j < 1 ? 1 : (j > tc.n_fj - 1 ? tc.n_fj - 1 : j);

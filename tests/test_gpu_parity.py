@@ -78,6 +78,7 @@ def check_toplist_complete(torch, d_counts, top, k, weighted):
     only): every template above the cut value is in the toplist, and the entries AT the cut are the lowest indices
     (unweighted: exactly; weighted: inside the 1e-5 band of the k-th value)."""
     vals = top["wcount"] if weighted else top["count"]
+    assert len(set(int(i) for i in top["index"][:k])) == k, "a template appears twice in the toplist"
     cut = vals[k - 1]
     d_cut = torch.tensor(cut, dtype=d_counts.dtype, device=d_counts.device)
     if weighted:
@@ -134,9 +135,31 @@ def test_empty_and_bad_arguments_are_rejected(bsh, torch, ctx):
     bad = dataclasses.replace(wl, k_band0=wl.k_slab0 - 1)
     with pytest.raises(bsh.BshError):
         ctx.stage1_hough(d_peak, bad)
+    far = dataclasses.replace(wl, k_band0=(1 << 32) - wl.n_f0, k_slab0=(1 << 32) - wl.n_f0 - 9)
+    with pytest.raises(bsh.BshError, match="2\\^32"):
+        ctx.stage1_hough(d_peak, far)                                  # band beyond the range the break fix-up is proven on (R-7)
     with pytest.raises(bsh.BshError):
         ctx._pending = (None, 4)                                       # collect without a pending launch
         ctx.stage1_collect()
+    # topk beyond the documented 2^27 is refused before anything is sized from it, even on a grid this small (the
+    # output pointers are never touched, so small dummies do)
+    import ctypes as C
+    pb = bsh.binding._Problem(wl, None)
+    dummy = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    n_top = C.c_int32(-5)
+    for topk in ((1 << 27) + 1, 2**31 - 1):
+        rc = ctx.lib.bsh_stage1_hough(ctx._ctx, C.c_void_p(d_peak.data_ptr()), C.c_int32(d_peak.shape[1]), C.byref(pb.sfts),
+                                      C.byref(pb.grid), C.c_int32(0), C.c_int32(topk), C.c_void_p(dummy.data_ptr()),
+                                      C.byref(n_top), None)
+        assert rc == -1 and b"2^27" in ctx.lib.bsh_last_error(ctx._ctx)
+        rho = np.ascontiguousarray(wl.rho, np.float32)
+        host_top = np.zeros(4, bsh.CAND_DTYPE)
+        rc = ctx.lib.bsh_search_patch_host(ctx._ctx, C.c_void_p(rho.ctypes.data), None, C.c_float(1.6), C.byref(pb.sfts),
+                                           C.byref(pb.grid), C.c_int32(0), C.c_int32(topk), C.c_void_p(host_top.ctypes.data),
+                                           C.byref(n_top))
+        assert rc == -1 and b"2^27" in ctx.lib.bsh_last_error(ctx._ctx) and not host_top["index"].any()
+    got, n = ctx.stage1_hough(d_peak, wl, topk=1 << 20)                  # far more than the 1620 templates: still fine
+    assert n == 1620
 
 
 # ------------------------------------------------------------------------------------------------------------
@@ -290,6 +313,7 @@ def _sampled_full_size_checks(bsh, torch, ctx, wl, weighted, n_sample=3000):
     pk = oracle.peakgram(wl.rho)
     top = r["top"]
     assert r["n_top"] == wl.topk
+    assert len(set(int(i) for i in top["index"])) == wl.topk, "a template appears twice in the toplist"
     n_o, w_o, _ = oracle.score(wl, top["index"], peak=pk, w=wl.w)
     assert np.array_equal(top["count"], n_o)
     assert np.allclose(top["wcount"], w_o, rtol=RTOL, atol=0)
@@ -635,6 +659,36 @@ def test_set_option_validates(bsh, torch, ctx):
     with pytest.raises(bsh.BshError):
         ctx.set_option(bsh.BSH_OPT_PIXELS_PER_THREAD, 3)
     ctx.set_option(bsh.BSH_OPT_KERNEL_FAMILY, bsh.BSH_FAMILY_AUTO)
+
+
+def test_outputs_live_on_the_contexts_device_and_stream(bsh, torch, ctx):
+    """Every buffer the binding hands to the library is allocated on the context's device under the context's stream
+    (ADVICE r2): a context bound to a side stream, used while torch's current stream is the default one, returns the same
+    results as the default-stream context, on the right device."""
+    side = torch.cuda.Stream()
+    c2 = bsh.Context(0, stream=side)
+    try:
+        wl = synth.config1()
+        d_rho = dev(torch, wl.rho)
+        torch.cuda.synchronize()
+        want = ctx.build_peakgram(d_rho)
+        got = c2.build_peakgram(d_rho)
+        side.synchronize()
+        assert got.device == d_rho.device and torch.equal(got, want)
+        cl = synth.candidate_list(3, n_background=200)
+        d = tuple(torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (cl.param, cl.res, cl.sig))
+        torch.cuda.synchronize()
+        a, b = ctx.post_cluster(d, 3.0), c2.post_cluster(d, 3.0)
+        assert all(torch.equal(a[k], b[k]) for k in ("label", "root", "centroid", "significance", "n_members")) and a["best"] == b["best"]
+        assert b["label"].device.index == 0
+        pa, pb = ctx.post_coincidences(d, d, 3.0), c2.post_coincidences(d, d, 3.0)
+        assert all(torch.equal(x, y) for x, y in zip(pa, pb)) and pb[0].device.index == 0
+        top_a, n_a = ctx.stage1_hough(want, wl)
+        top_b, n_b = c2.stage1_hough(got, wl)
+        side.synchronize()
+        assert n_a == n_b and torch.equal(top_a, top_b)
+    finally:
+        c2.close()
 
 
 def test_measured_peaks_are_plausible(bsh, torch, ctx):
