@@ -130,3 +130,10 @@ def test_eccentric_large_toplist_paths(bsh, torch, ctx):
     w, topw = run(bsh, torch, ctx, wl, bsh.BSH_WEIGHTED, topk=100_000)
     assert np.array_equal(topw["count"], want_n[topw["index"].astype(np.int64)])
     assert np.all(np.diff(topw["wcount"]) <= 0)
+    assert np.allclose(w, want_w, rtol=RTOL, atol=0)                                  # every weighted count of the grid
+    assert np.allclose(topw["wcount"], want_w[topw["index"].astype(np.int64)], rtol=RTOL, atol=0)
+    assert len(set(int(i) for i in topw["index"])) == 100_000
+    # the weighted toplist is the top 100 000 of the oracle's weighted counts up to ties within the tolerance at the cut
+    cut = np.sort(want_w)[::-1][100_000 - 1]
+    assert set(np.nonzero(want_w > cut * (1 + RTOL))[0].tolist()) <= set(int(i) for i in topw["index"])
+    assert np.all(want_w[topw["index"].astype(np.int64)] >= cut * (1 - RTOL))
