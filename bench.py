@@ -175,15 +175,17 @@ def run_oracle_steps(wl, label, steps: int, warmup: int, seconds_per_step: float
 
 def cpu_baseline(wl, label):
     """All host cores (~12 s) and one thread (~6 s), same oracle, same inputs; extrapolation flagged as such."""
-    value, _, cores, sample = run_oracle_steps(wl, label, 1, 0, seconds_per_step=12.0)
-    v1, _, _, sample1 = run_oracle_steps(wl, label, 1, 0, seconds_per_step=6.0, n_threads=1)
     import oracle
+    all_threads = oracle.max_threads()                  # read BEFORE the single-thread leg: that leg's omp_set_num_threads(1)
+    value, _, cores, sample = run_oracle_steps(wl, label, 1, 0, seconds_per_step=12.0)   # is process-wide and would otherwise
+    v1, _, _, sample1 = run_oracle_steps(wl, label, 1, 0, seconds_per_step=6.0, n_threads=1)   # leave the tier-2 leg on 1 thread
     pk = oracle.peakgram(wl.rho)
     sub2 = wl.subgrid(ia=[0], ip=list(range(min(6, len(wl.P)))))
     t0 = time.perf_counter()
-    oracle.tier2_stage1(sub2, pk)
+    oracle.tier2_stage1(sub2, pk, n_threads=all_threads)
     dt2 = time.perf_counter() - t0
-    tier2 = {"value": sub2.n_accumulations / dt2, "unit": UNIT, "cores": oracle.max_threads(),
+    assert oracle.max_threads() == all_threads
+    tier2 = {"value": sub2.n_accumulations / dt2, "unit": UNIT, "cores": all_threads,
              "kind": "tier-2 CPU reference (oracle/bsh_tier2.c): the same track-sharing math as the GPU path -- one track "
                      "evaluation per (pixel, binary template, SFT), bytes of the band added by a vector loop",
              "sample": f"{sub2.n_pix} pixels x {sub2.n_binary} binary templates x {sub2.n_f0} f0 x {sub2.n_sft} SFTs = "
