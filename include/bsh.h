@@ -37,8 +37,8 @@ extern "C" {
 #define BSH_ENOMEM   -2   /* device or host allocation failed                                                    */
 #define BSH_ECUDA    -3   /* a CUDA runtime call or kernel failed (message in bsh_last_error)                    */
 #define BSH_ESMALL   -4   /* an output buffer is too small (e.g. words_per_row * 32 < n_bins)                    */
-#define BSH_ESTATE   -5   /* call order violated (e.g. bsh_stage1_collect without bsh_stage1_launch), or the candidate  */
-                          /* selection did not converge (degenerate input); message in bsh_last_error              */
+#define BSH_ESTATE   -5   /* call order violated (e.g. bsh_stage1_collect without bsh_stage1_launch), or the threshold   */
+                          /* search of the toplist gave up after 24 accumulation passes; message in bsh_last_error */
 #define BSH_ELIMIT   -6   /* a list is longer than the fixed scratch of bsh_post_coincidences_static holds               */
 
 /* mode bits for stage 1 */
@@ -187,6 +187,13 @@ double bsh_median_bias(int32_t window);    /* sum_{i = (window + 1) / 2}^{window
  *   d_counts_full   optional dump of the ranking statistic of EVERY template (int32 counts in BSH_UNWEIGHTED mode,
  *                   float weighted counts in BSH_WEIGHTED mode), [n_templates]; NULL in production
  * A track leaving the slab is not an error: that SFT contributes 0 (R-6).
+ * Toplist selection: the accumulation kernels emit the templates at or above a threshold guessed from noise moments of the
+ * peakgram into a candidate buffer (2^20 entries, more for topk > 2^17), which is then sorted.  When the data are not noise-
+ * like and fewer than topk or more than the buffer holds pass, the accumulation is repeated with a corrected threshold
+ * (bsh_stats.n_passes > 1): lowered in doubling steps, or raised to the topk-th value of the overflowed buffer.  When the
+ * templates tied AT the cut value alone overflow the buffer (all-zero or constant peakgram rows, very few SFTs), the ties
+ * are admitted in template-index order up to a limit found by a few more passes, so the result is still exactly the
+ * (statistic desc, index asc) toplist.  Grids that fit the buffer are emitted whole and never need this.
  * bsh_stage1_hough = bsh_stage1_launch + bsh_stage1_collect; it returns with d_top complete (stream synchronised).
  * bsh_stage1_launch is asynchronous (no host synchronisation); bsh_stage1_collect synchronises the stream, runs the
  * selection, and leaves the toplist writes enqueued on the stream (h_n_top is final on return).  The wcount of every

@@ -29,7 +29,7 @@ using namespace bsh;
 namespace {
 
 constexpr unsigned int kCandCap = 1u << 20;      // candidate buffer entries (16 MB)
-constexpr int kMaxPasses = 12;
+constexpr int kMaxPasses = 24;               // accumulation passes per call, all phases of the threshold search together
 constexpr int32_t kMaxTopk = 1 << 27;            // bsh.h: 1 <= topk <= 2^27 (also the largest candidate buffer)
 
 struct DevBuf {
@@ -62,8 +62,17 @@ struct Pending {                      // state between bsh_stage1_launch and bsh
     int tile_bins = 96;               // f0 bins per accumulation pass (<= 32 NW)
     unsigned int cand_cap = kCandCap; // candidate buffer entries of this call (grows with topk: fraction-N_C toplists, L225)
     int R = 2, NW = 3, HP = 6, n_entries = 0, off_table = 0, s_max = 0, s_zero = 0, list_cap = 0, tpb = 256, n_groups = 0, n_aq_tiles = 0;
-    double frac = 0, shift_sigma = 0;
+    double frac = 0;
     int passes = 0;
+    // threshold search of bsh_stage1_collect (passes after the first run with a host-given threshold)
+    bool fixed = false;               // false: the noise-model threshold of threshold_kernel (first pass)
+    double tau = 0;                   // the threshold of the pass in flight (integer-valued in unweighted mode)
+    double lo_tau = 0;                // the last threshold with too many survivors ...
+    uint64_t lo_n = 0;                // ... and how many there were
+    double step_dn = 0.75;
+    int phase = 0;                    // 0: search on tau; 1: count the templates above the tie value; 2: search on tie_limit
+    uint64_t tie_limit = ~0ull, lim_lo = 0, lim_hi = 0, n_above = 0;
+    uint32_t tie_key = 0;
     // position-table kernels (bsh_pos.cuh)
     bool use_pos = false;
     int pos_off = 0, pos_s_max = 0, pos_s_zero = 0, n_pos = 0, n_stages = 0, n_oct = 0, pos_groups = 0, pos_smem = 0;
@@ -428,8 +437,9 @@ int run_pass(bsh_ctx *ctx)
     const TableCache &c = ctx->cache[pd.cache_slot];
     const bool weighted = (pd.mode & BSH_WEIGHTED) != 0;
     CK(cudaMemsetAsync(ctx->cand_count.p, 0, sizeof(unsigned int), ctx->stream));
-    threshold_kernel<<<1, 1, 0, ctx->stream>>>((const double *)ctx->stats.p, pd.frac, pd.shift_sigma, pd.emit_all ? 1 : 0,
-                                               (Threshold *)ctx->thr.p);
+    threshold_kernel<<<1, 1, 0, ctx->stream>>>((const double *)ctx->stats.p, pd.frac, pd.emit_all ? 1 : 0, pd.fixed ? 1 : 0,
+                                               (int32_t)std::max(-1.0e9, std::min(1.0e9, pd.tau)), (float)pd.tau, pd.tie_key,
+                                               pd.tie_limit, (Threshold *)ctx->thr.p);
     count_launch(ctx);
     CK(cudaEventRecord(ctx->ev[2], ctx->stream));
     if (pd.mode & BSH_NAIVE) {
@@ -961,7 +971,6 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     pd.frac = (double)std::max<int64_t>(8ll * topk, 4096) / (double)pd.n_templates;
     if ((uint64_t)topk > kCandCap / 8) pd.frac = (1.3 * (double)topk + 4096.0) / (double)pd.n_templates;
     if (pd.frac >= 0.25) pd.frac = (uint64_t)topk > kCandCap / 8 ? std::min(pd.frac, 0.45) : 0.25;
-    pd.shift_sigma = 0.0;
     pd.passes = 0;
 
     // device scratch
@@ -1042,7 +1051,7 @@ int bsh_stage1_launch(bsh_ctx *ctx, const uint32_t *d_peak, int32_t words_per_ro
     TRY(run_pass(ctx));
     ctx->have_kernel = true;
     CK(cudaMemcpyAsync(ctx->pinned_count, ctx->cand_count.p, sizeof(unsigned int), cudaMemcpyDeviceToHost, ctx->stream));
-    CK(cudaMemcpyAsync(ctx->pinned_count + 4, ctx->thr.p, sizeof(Threshold), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->pinned_count + 4, ctx->thr.p, kThresholdHostBytes, cudaMemcpyDeviceToHost, ctx->stream));
     ctx->pend.active = true;
 
     ctx->st.n_templates = (int64_t)pd.n_templates;
@@ -1061,29 +1070,94 @@ int bsh_stage1_collect(bsh_ctx *ctx, bsh_cand *d_top, int32_t *h_n_top)
     const bool weighted = (pd.mode & BSH_WEIGHTED) != 0;
     const uint64_t want = std::min<uint64_t>((uint64_t)pd.topk, pd.n_templates);
     unsigned int n_cand = 0;
+    Threshold thr = {};
+    // Threshold search.  The first pass used the noise-model threshold.  Too few survivors (< topk) or too many (> the
+    // candidate buffer) happen when the data are not what the model assumes (lines, notched bands, constant rows).  Then:
+    //   too few    lower tau by steps that double (0.75, 1.5, 3 ... model sigmas), not below 0 (both statistics are >= 0).
+    //   too many   the buffer holds cand_cap of the survivors; its topk-th largest value T_b has at least topk templates at
+    //              or above it, so tau = T_b cannot give too few and normally lands in range at once.  T_b equal to the
+    //              threshold itself means that the templates AT that value alone overflow the buffer -- massive ties at
+    //              the cut (notched band, constant rows, very few SFTs):
+    //   phase 1    count the templates above the tie value T (one pass at the next representable threshold);
+    //   phase 2    tau = T, and of the ties only those with template index < tie_limit are emitted; search on tie_limit
+    //              (first guess from the tie density, then regula falsi / bisection).  The buffer then holds everything
+    //              above T and the lowest-index ties, which contains the (value desc, index asc) toplist.
     for (;;) {
         CK(cudaStreamSynchronize(ctx->stream));
         n_cand = ctx->pinned_count[0];
+        memcpy(&thr, ctx->pinned_count + 4, kThresholdHostBytes);
+        if (!pd.fixed) pd.tau = weighted ? (double)thr.tau_f : (double)thr.tau_i;
         const bool too_few = n_cand < want, too_many = n_cand > pd.cand_cap;
         if (!too_few && !too_many) break;
         if (pd.passes >= kMaxPasses)
-            return fail(ctx, BSH_ESTATE, "candidate selection did not converge after %d passes (%u candidates for topk %d; degenerate "
-                                         "input: constant rows or massive ties at the cut?)", pd.passes, n_cand, pd.topk);
+            return fail(ctx, BSH_ESTATE, "candidate selection did not converge after %d passes (%u candidates for topk %d at "
+                                         "threshold %g, phase %d)", pd.passes, n_cand, pd.topk, pd.tau, pd.phase);
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, ctx->ev[2], ctx->ev[3]) == cudaSuccess) ctx->kernel_ms_extra += ms;
-        if (too_few) {
-            pd.shift_sigma -= 0.75;
-            if (pd.passes >= 6 && pd.n_templates <= pd.cand_cap) pd.emit_all = true;   // (else emit_all would overflow the buffer)
-        } else {
-            pd.emit_all = false;
-            pd.shift_sigma += 0.5;
+        const double sigma = (double)thr.sigma, mean = (double)thr.mean;
+        const double unit = sigma > 0.0 ? sigma : (weighted ? std::max(fabs(mean) * 0.01, 1.0e-3) : 1.0);
+        auto next_up = [&](double t) { return weighted ? (double)nextafterf((float)t, INFINITY) : t + 1.0; };
+        bool start_ties = false;
+        if (pd.phase == 1 && too_many) pd.phase = 0;                  // not ties after all: an ordinary overflow
+        if (pd.phase == 0 && too_many) {
+            TRY(ensure(ctx, ctx->keys, (size_t)pd.cand_cap * sizeof(RawCand)));
+            RawCand *by_value = nullptr;
+            TRY(radix_sort_candidates(ctx, (RawCand *)ctx->cand.p, (RawCand *)ctx->keys.p, pd.cand_cap, &by_value));
+            CK(cudaMemcpyAsync(ctx->pinned_count + 2, &by_value[want - 1].key, 4, cudaMemcpyDeviceToHost, ctx->stream));
+            CK(cudaStreamSynchronize(ctx->stream));
+            const uint32_t kb = ctx->pinned_count[2];
+            float fb;
+            memcpy(&fb, &kb, 4);
+            const double t_b = weighted ? (double)fb : (double)kb;
+            pd.lo_tau = std::max(pd.tau, 0.0);
+            pd.lo_n = n_cand;
+            if (t_b > pd.lo_tau) {
+                pd.tau = t_b;
+            } else {
+                pd.phase = 1;
+                pd.tau = next_up(pd.lo_tau);
+            }
+        } else if (pd.phase == 0) {                                   // too few
+            double t = weighted ? (double)(float)(pd.tau - pd.step_dn * unit) : floor(pd.tau - pd.step_dn * unit);
+            if (t >= pd.tau) t = weighted ? (double)nextafterf((float)pd.tau, -INFINITY) : pd.tau - 1.0;
+            if (pd.tau <= 0.0)
+                return fail(ctx, BSH_ESTATE, "fewer than topk = %d of the %llu templates pass a threshold of zero", pd.topk,
+                            (unsigned long long)pd.n_templates);
+            pd.tau = t > 0.0 ? t : 0.0;
+            pd.step_dn *= 2.0;
+        } else if (pd.phase == 1) {                                   // this pass ran just above the tie value: too few
+            pd.n_above = n_cand;
+            start_ties = true;
+        } else {                                                      // phase 2: this pass ran with pd.tie_limit
+            if (too_few) pd.lim_lo = pd.tie_limit; else pd.lim_hi = pd.tie_limit;
+            const double got = (double)n_cand - (double)pd.n_above;   // ties below the limit
+            const double need = 1.5 * (double)(want - pd.n_above) + 64.0;
+            double guess = got > 0.0 ? (double)pd.tie_limit * need / got : (double)pd.tie_limit * 16.0;
+            const double lo = (double)pd.lim_lo, hi = (double)pd.lim_hi;
+            if (!(guess > lo + 0.05 * (hi - lo) && guess < hi - 0.05 * (hi - lo))) guess = 0.5 * (lo + hi);
+            if (pd.lim_hi - pd.lim_lo <= 1)
+                return fail(ctx, BSH_ESTATE, "tie-limit search collapsed at %llu (%u candidates for topk %d)",
+                            (unsigned long long)pd.tie_limit, n_cand, pd.topk);
+            pd.tie_limit = std::min<uint64_t>(pd.lim_hi - 1, std::max<uint64_t>(pd.lim_lo + 1, (uint64_t)guess));
+        }
+        pd.fixed = true;
+        if (start_ties) {
+            pd.phase = 2;
+            pd.tau = pd.lo_tau;
+            const float tf = (float)pd.lo_tau;
+            uint32_t key;
+            if (weighted) memcpy(&key, &tf, 4); else key = (uint32_t)(int32_t)pd.lo_tau;
+            pd.tie_key = key;
+            pd.lim_lo = 0;
+            pd.lim_hi = pd.n_templates;
+            const double n_tie = (double)pd.lo_n - (double)pd.n_above;            // templates AT the tie value
+            const double need = 1.5 * (double)(want - pd.n_above) + 64.0;
+            pd.tie_limit = (uint64_t)std::min((double)pd.n_templates - 1.0, std::max(1.0, (double)pd.n_templates * need / std::max(n_tie, 1.0)));
         }
         TRY(run_pass(ctx));
         CK(cudaMemcpyAsync(ctx->pinned_count, ctx->cand_count.p, sizeof(unsigned int), cudaMemcpyDeviceToHost, ctx->stream));
-        CK(cudaMemcpyAsync(ctx->pinned_count + 4, ctx->thr.p, sizeof(Threshold), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaMemcpyAsync(ctx->pinned_count + 4, ctx->thr.p, kThresholdHostBytes, cudaMemcpyDeviceToHost, ctx->stream));
     }
-    Threshold thr;
-    memcpy(&thr, ctx->pinned_count + 4, sizeof thr);
     ctx->st.n_candidates = n_cand;
     ctx->st.threshold = weighted ? (double)thr.tau_f : (double)thr.tau_i;
     ctx->st.n_passes = pd.passes;

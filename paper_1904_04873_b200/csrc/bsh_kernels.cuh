@@ -176,22 +176,56 @@ __global__ void __launch_bounds__(256) prep_table_kernel(const uint32_t *__restr
 struct Threshold {
     int32_t tau_i;      // unweighted: emit when count >= tau_i
     float tau_f;        // weighted:   emit when n_w   >= tau_f
-    float mean, sigma;  // of the noise model
+    float mean, sigma;  // of the noise model                                   (the host reads back these first 16 bytes)
+    // Massive ties at the cut (more templates AT the k-th value than the candidate buffer holds: a cleaned / notched band,
+    // constant rows, very few SFTs): of the templates whose statistic has exactly the bit pattern tie_key only those with
+    // template index < tie_limit are candidates -- the order is (value desc, index asc), so the lowest indices are the
+    // ones a toplist can need.  A normal pass has tie_limit = 2^64 - 1: nothing is held back.
+    uint32_t tie_key;
+    uint32_t pad;
+    uint64_t tie_limit;
 };
+constexpr size_t kThresholdHostBytes = 16;
 
-// tau = mean + z sigma with z from the normal tail for the wanted survivor fraction, minus a safety margin; the host
-// lowers it and re-runs in the rare case fewer than topk templates pass (stats -> n_passes).
-__global__ void threshold_kernel(const double *__restrict__ stats, double frac, double shift_sigma, int emit_all,
-                                 Threshold *__restrict__ out)
+// First pass: tau = mean + z sigma with z from the normal tail for the wanted survivor fraction, minus a safety margin.
+// When too few or too many templates pass, the host (bsh_stage1_collect) searches for the threshold and re-runs with
+// fixed != 0: tau_i / tau_f / tie_key / tie_limit as given (stats -> n_passes).
+__global__ void threshold_kernel(const double *__restrict__ stats, double frac, int emit_all, int fixed, int32_t fixed_tau_i,
+                                 float fixed_tau_f, uint32_t tie_key, uint64_t tie_limit, Threshold *__restrict__ out)
 {
     const double mean = stats[0], sigma = sqrt(stats[1] > 0.0 ? stats[1] : 0.0);
     double z = -1.0e30;
-    if (!emit_all && frac < 0.5) z = -normcdfinv(frac) - 0.4 + shift_sigma;
+    if (!emit_all && frac < 0.5) z = -normcdfinv(frac) - 0.4;
     const double tau = emit_all ? -1.0e30 : mean + z * sigma;
     out->mean = (float)mean;
     out->sigma = (float)sigma;
     out->tau_f = tau < -1.0e29 ? -3.0e38f : (float)tau;
     out->tau_i = tau < -1.0e29 ? -(1 << 30) : (int32_t)floor(tau);
+    if (fixed && !emit_all) {
+        out->tau_f = fixed_tau_f;
+        out->tau_i = fixed_tau_i;
+    }
+    out->tie_key = tie_key;
+    out->pad = 0u;
+    out->tie_limit = tie_limit;
+}
+
+// A template that passed the threshold goes into the candidate buffer (key = the count, or the bits of the FP32 weighted
+// count) -- unless it is one of the ties held back by tie_limit.  cand_count counts every survivor, also those beyond the
+// buffer's capacity: the host sees the overflow there.
+__device__ __noinline__ void emit_survivor(const Threshold *__restrict__ thr, RawCand *__restrict__ cand,
+                                              unsigned int *__restrict__ cand_count, unsigned int cand_cap, uint64_t index,
+                                              uint32_t key)
+{
+    if (key == thr->tie_key && index >= thr->tie_limit) return;
+    const unsigned int pos = atomicAdd(cand_count, 1u);
+    if (pos < cand_cap) {
+        RawCand rc;
+        rc.index = index;
+        rc.key = key;
+        rc.pad = 0u;
+        cand[pos] = rc;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -288,14 +322,7 @@ __device__ __forceinline__ TrackConst make_track_const(const Stage1Params &p, co
 
 __device__ __forceinline__ void emit_candidate(const Stage1Params &p, uint64_t index, uint32_t key)
 {
-    const unsigned int pos = atomicAdd(p.cand_count, 1u);
-    if (pos < p.cand_cap) {
-        RawCand rc;
-        rc.index = index;
-        rc.key = key;
-        rc.pad = 0u;
-        p.cand[pos] = rc;
-    }
+    emit_survivor(p.thr, p.cand, p.cand_count, p.cand_cap, index, key);
 }
 
 // Shared-memory staging of one chunk of kChunk SFTs: window-table rows, (cos, sin) rows of this period, D rows of this
@@ -632,16 +659,7 @@ __global__ void __launch_bounds__(256) stage1_naive_kernel(const TrackTables t, 
         pass = n >= thr->tau_i;
         key = (uint32_t)n;
     }
-    if (pass) {
-        const unsigned int pos = atomicAdd(cand_count, 1u);
-        if (pos < cand_cap) {
-            RawCand rc;
-            rc.index = idx;
-            rc.key = key;
-            rc.pad = 0u;
-            cand[pos] = rc;
-        }
-    }
+    if (pass) emit_survivor(thr, cand, cand_count, cand_cap, idx, key);
 }
 
 // ---------------------------------------------------------------------------------------------------------------------

@@ -482,14 +482,7 @@ __global__ void __launch_bounds__(32 * kPixWarps, BSH_PIX_MINB) stage1_unweighte
             while (m) {
                 const int bb = __ffs(m) - 1;
                 m &= m - 1;
-                const unsigned int pos = atomicAdd(p.cand_count, 1u);
-                if (pos < p.cand_cap) {
-                    RawCand rc;
-                    rc.index = base + 32 * w + bb;
-                    rc.key = (uint32_t)count_at(full_cnt, w, bb);
-                    rc.pad = 0u;
-                    p.cand[pos] = rc;
-                }
+                emit_survivor(p.thr, p.cand, p.cand_count, p.cand_cap, base + 32 * w + bb, (uint32_t)count_at(full_cnt, w, bb));
             }
         }
     }

@@ -339,14 +339,7 @@ __global__ void __launch_bounds__(32 * kWarpsUnweighted, 2) stage1_unweighted_po
             while (m) {
                 const int b = __ffs(m) - 1;
                 m &= m - 1;
-                const unsigned int pos = atomicAdd(p.cand_count, 1u);
-                if (pos < p.cand_cap) {
-                    RawCand rc;
-                    rc.index = base + 32 * w + b;
-                    rc.key = (uint32_t)count_at(cnt[r], w, b);
-                    rc.pad = 0u;
-                    p.cand[pos] = rc;
-                }
+                emit_survivor(p.thr, p.cand, p.cand_count, p.cand_cap, base + 32 * w + b, (uint32_t)count_at(cnt[r], w, b));
             }
         }
     }
@@ -443,14 +436,7 @@ __global__ void __launch_bounds__(32 * kWarpsWeighted, 2) stage1_weighted_pos_ke
             if (j < p.n_fj) {
                 if (out) out[j] = acc[j];
                 if (acc[j] >= tau) {
-                    const unsigned int pos = atomicAdd(p.cand_count, 1u);
-                    if (pos < p.cand_cap) {
-                        RawCand rc;
-                        rc.index = base + j;
-                        rc.key = __float_as_uint(acc[j]);
-                        rc.pad = 0u;
-                        p.cand[pos] = rc;
-                    }
+                    emit_survivor(p.thr, p.cand, p.cand_count, p.cand_cap, base + j, __float_as_uint(acc[j]));
                 }
             }
         }

@@ -435,14 +435,7 @@ __global__ void __launch_bounds__(32 * kWpixWarps, kWpixBlocksPerSm) stage1_weig
             if (j < p.n_fj) {
                 if (out) out[j] = acc[j];
                 if (acc[j] >= tau) {
-                    const unsigned int pos = atomicAdd(p.cand_count, 1u);
-                    if (pos < p.cand_cap) {
-                        RawCand rc;
-                        rc.index = base + j;
-                        rc.key = __float_as_uint(acc[j]);
-                        rc.pad = 0u;
-                        p.cand[pos] = rc;
-                    }
+                    emit_survivor(p.thr, p.cand, p.cand_count, p.cand_cap, base + j, __float_as_uint(acc[j]));
                 }
             }
         }
