@@ -213,7 +213,7 @@ __global__ void threshold_kernel(const double *__restrict__ stats, double frac, 
 // A template that passed the threshold goes into the candidate buffer (key = the count, or the bits of the FP32 weighted
 // count) -- unless it is one of the ties held back by tie_limit.  cand_count counts every survivor, also those beyond the
 // buffer's capacity: the host sees the overflow there.
-__device__ __noinline__ void emit_survivor(const Threshold *__restrict__ thr, RawCand *__restrict__ cand,
+__device__ __forceinline__ void emit_survivor(const Threshold *__restrict__ thr, RawCand *__restrict__ cand,
                                               unsigned int *__restrict__ cand_count, unsigned int cand_cap, uint64_t index,
                                               uint32_t key)
 {
@@ -318,6 +318,18 @@ __device__ __forceinline__ TrackConst make_track_const(const Stage1Params &p, co
     tc.s_zero = p.s_zero;
     tc.n_fj = p.n_fj;
     return tc;
+}
+
+// The same, compiled out of line, for the weighted pixel-lane kernel (bsh_wpix.cuh): its epilogue tests 90 accumulators one
+// after the other, and 90 inlined copies of the emission cost the kernel 10 registers and 296 bytes of spills in the hot
+// loop (168 -> 158 registers, none spilled; config 3: 730 -> 644 ms per launch, profiles/r03_stage1_wpix_full.md).  The
+// unweighted kernels keep the inline form: they lose nothing to it, and a toplist of a fraction N_C of the bank (L225)
+// emits millions of survivors, where a call per survivor costs (27.8 -> 36.0 ms on the N_C = 5 % pass of config 2).
+__device__ __noinline__ void emit_survivor_out_of_line(const Threshold *__restrict__ thr, RawCand *__restrict__ cand,
+                                                       unsigned int *__restrict__ cand_count, unsigned int cand_cap,
+                                                       uint64_t index, uint32_t key)
+{
+    emit_survivor(thr, cand, cand_count, cand_cap, index, key);
 }
 
 __device__ __forceinline__ void emit_candidate(const Stage1Params &p, uint64_t index, uint32_t key)

@@ -435,7 +435,7 @@ __global__ void __launch_bounds__(32 * kWpixWarps, kWpixBlocksPerSm) stage1_weig
             if (j < p.n_fj) {
                 if (out) out[j] = acc[j];
                 if (acc[j] >= tau) {
-                    emit_survivor(p.thr, p.cand, p.cand_count, p.cand_cap, base + j, __float_as_uint(acc[j]));
+                    emit_survivor_out_of_line(p.thr, p.cand, p.cand_count, p.cand_cap, base + j, __float_as_uint(acc[j]));
                 }
             }
         }
