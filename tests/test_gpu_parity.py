@@ -383,7 +383,7 @@ def test_config2_full_grid_against_the_tier2_cpu_reference(bsh, torch, ctx):
 
 def test_config3_slice_config4_and_config5_patch_against_the_tier2_cpu_reference(bsh, torch, ctx):
     """Full grids of a config-4 patch and a config-5 patch, and a 10 % slice (4 of the 40 a_p values) of the full-size
-    config-3 run, against the tier-2 CPU reference."""
+    config-3 run -- integer counts and the FP32 weighted counts of the headline mode -- against the tier-2 CPU reference."""
     # config 3: the GPU runs the FULL grid in the bench launch configuration; the slice of its dump is compared
     wl = synth.config3()
     pk = oracle.peakgram(wl.rho)
@@ -396,7 +396,19 @@ def test_config3_slice_config4_and_config5_patch_against_the_tier2_cpu_reference
     per_ap = len(wl.P) * len(wl.tasc_frac) * wl.n_f0
     got = d_counts.view(wl.n_pix, len(wl.ap), per_ap)[:, ia, :].contiguous().view(-1).cpu().numpy()
     assert np.array_equal(got, n_ref)
-    del d_counts
+    del d_counts, got
+    # the headline mode at the headline size: the WEIGHTED FP32 counts of the same full-size run, one a_p value of the
+    # grid (4.1e7 templates, every one compared) against the tier-2 reference's FP64 weighted counts (its FP64 weighted
+    # path is ~10x slower than its integer one: a 4-value slice would double the run time of the whole GPU suite)
+    ia = [26]
+    _, w_ref = oracle.tier2_stage1(wl.subgrid(ia=ia), pk, wl.w, want_wcount=True)
+    d_wcounts = torch.full((wl.n_templates,), -7.0, dtype=torch.float32, device="cuda")
+    ctx.stage1_hough(d_peak, wl, mode=bsh.BSH_WEIGHTED, topk=wl.topk, d_w=d_w, counts_full=d_wcounts)
+    assert ctx.stats()["kernel_variant"] // 1000 == 3, "the weighted pixel-lane kernel did not run"
+    got_w = d_wcounts.view(wl.n_pix, len(wl.ap), per_ap)[:, ia, :].contiguous().view(-1).cpu().numpy()
+    del d_wcounts
+    assert got_w.shape == w_ref.shape and np.allclose(got_w, w_ref, rtol=RTOL, atol=0)
+    del got_w, w_ref
     # config 4, patch 0 (with its injection), from |x|^2
     c4 = synth.config4()
     inj = c4.injections[0]
